@@ -1,0 +1,154 @@
+/*
+ * gramsci.h -- C ABI of the B200-native GRAMSCI-style N-point correlation query engine.
+ *
+ * Citations: P:<n> = PAPER.md line n (arxiv/paper_2607_06604); S:8(c) A-k = SURVEY.md section 8(c)
+ * reading k (all restated in DESIGN.md section 3).
+ *
+ * The library computes, on one CUDA device (sm_100a), binned counts of the 2-, 3- and 4-cliques of
+ * the radius graph of a point catalogue, and the parity-decomposed 4-clique counts
+ * (P:91-101).  Every step runs in hand-written CUDA kernels; there is no CPU fallback: a call on a
+ * machine without a usable CUDA device returns GRAMSCI_ECUDA.
+ *
+ * POINTERS.  Every data pointer (points, weights, output histograms) may be a DEVICE pointer or a
+ * HOST pointer (pageable or pinned); the library asks the CUDA runtime which one it was given
+ * (cudaPointerGetAttributes) and stages host buffers through device scratch itself.  `box` and all
+ * scalar out-parameters are always HOST pointers.
+ *
+ * OWNERSHIP.  The caller owns points, weights and every output buffer.  The library owns the graph
+ * (opaque handle) and all scratch, and releases them in gramsci_free_graph.  points/weights may be
+ * freed as soon as gramsci_build_graph returns (weights are copied, coordinates discarded).
+ *
+ * OUTPUTS are overwritten (not accumulated) and are complete when the call returns (the call
+ * enqueues on the graph's stream and synchronises that stream before returning).  Any output
+ * pointer may be NULL to skip that channel.  Layout: dense row-major [nb]^3, index (b1*nb+b2)*nb+b3
+ * or [nb]^6 in the order (b12,b13,b14,b23,b24,b34); populated ONLY at canonical configurations
+ * (3pCF: sorted triple b1<=b2<=b3, A-5; 4pCF: lexicographic minimum over the 24 vertex orders, A-7),
+ * zero elsewhere.
+ *
+ * ERRORS.  Every function returns a gramsci_status; nothing throws or aborts across the ABI; on
+ * failure no output is written.  gramsci_last_error() gives a thread-local message.
+ *
+ * DETERMINISM.  Unweighted counts are exact integers, identical run to run and with or without a
+ * device-memory cap.  Weighted fp64 sums may differ in the last bits with atomic order.
+ */
+#ifndef GRAMSCI_H
+#define GRAMSCI_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gramsci_graph gramsci_graph; /* opaque, owned by the library */
+
+typedef enum {
+    GRAMSCI_OK = 0,
+    GRAMSCI_EINVAL = 1,    /* bad pointer / size / nbins / radii / unsupported combination         */
+    GRAMSCI_ERANGE = 2,    /* periodic box with r_max >= min(box)/2 (A-4), or a row too long for smem */
+    GRAMSCI_ENOMEM = 3,    /* device or host allocation failed, or device_mem_cap_bytes too small    */
+    GRAMSCI_ECUDA = 4,     /* CUDA runtime error, or no CUDA device (see gramsci_last_error)         */
+    GRAMSCI_EOVERFLOW = 5  /* N >= 2^31                                                              */
+} gramsci_status;
+
+/* 3pCF intersection kernel variants (S:8(f) rank 2 ablation). 0 picks the default. */
+enum {
+    GRAMSCI_ALGO_DEFAULT = 0,
+    GRAMSCI_ALGO_MERGEPATH = 1, /* merge-path partitioned two-list intersection (P:57-70 on a warp) */
+    GRAMSCI_ALGO_BSEARCH = 2,   /* lane-parallel binary search of N+(j) in the hub tail */
+    GRAMSCI_ALGO_BITMAP = 3     /* hub row scattered into a shared-memory slot table, O(1) membership */
+};
+
+typedef struct {       /* zero-initialised struct == defaults */
+    void *stream;                  /* cudaStream_t to run on (e.g. torch's current stream); NULL = default stream */
+    uint64_t device_mem_cap_bytes; /* 0 = keep the whole CSR resident; else the edge arrays live in pinned
+                                      host memory and are streamed through device windows of at most this
+                                      many bytes in total (out-of-core tiler)                   */
+    int want_pixels;               /* 1 = also store the direction-pixel byte per edge (needed by
+                                      gramsci_4pcf_parity); forces caller-label order (A-10)         */
+    int relabel;                   /* 0 = default (spatial relabelling unless want_pixels), 1 = force
+                                      spatial (cell-order) labels, 2 = force caller labels                 */
+    int algo;                      /* GRAMSCI_ALGO_* for gramsci_3pcf                                      */
+    int n_windows;                 /* out-of-core only: force this many row windows (0 = derive from cap);
+                                      the paper's env-var override, P:159                                 */
+} gramsci_options;
+
+/*
+ * Build the radius graph (S:8(a) A1-A5): edge {i,j} iff r_min <= d(i,j) < r_max (A-2), d the
+ * Euclidean distance, minimum image per axis when periodic (A-4).  Stored oriented (each edge once,
+ * at its lower internal label, A-15) as CSR: ptr int64 [N+1], idx int32 [E] sorted ascending within a
+ * row (Eq. 1), bin uint8 [E] = index of the equal-width bin of [r_min,r_max) (A-3: squared
+ * distances compared with squared bin edges, no FMA contraction), pix uint8 [E] (A-8) if want_pixels.
+ *
+ *   points   [N,3] fp64 row-major x,y,z; inside [0,box) per axis when periodic.   HOST or DEVICE.
+ *   weights  [N] fp64 (any sign) or NULL = unit weights.                            HOST or DEVICE.
+ *   box      HOST double[3] periodic side lengths; NULL or any entry <= 0 = open (non-periodic).
+ *   nbins    1..255 (bin index is one byte).
+ * Errors: EINVAL (NULL points with N>0, nbins, r_min<0, r_max<=r_min), ERANGE (r_max >= box/2),
+ * EOVERFLOW (N >= 2^31), ENOMEM, ECUDA.  On error *out is NULL.
+ */
+int gramsci_build_graph(const double *points, const double *weights, int64_t N, const double *box,
+                        double r_min, double r_max, int nbins, const gramsci_options *opt,
+                        gramsci_graph **out);
+
+/* Sizes of a built graph (all out-pointers HOST, any may be NULL). csr_bytes = 5E (+E with pixels). */
+int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edges, int32_t *max_row,
+                       uint64_t *csr_bytes, int32_t *n_windows);
+
+/*
+ * Copy the CSR out in CALLER labels (for graph-level parity tests): row i = caller point i, holding
+ * the caller labels j > i of its neighbours, ascending.  ptr int64 [N+1], idx int32 [E], bin uint8 [E],
+ * pix uint8 [E] (only if built with want_pixels, else untouched).  HOST or DEVICE; any may be NULL.
+ * With spatial relabelling the library converts (re-orients and re-sorts) on the device.
+ */
+int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t *idx, uint8_t *bin, uint8_t *pix);
+
+/* 2pCF sweep (S:8(a) A6): counts[b] = #edges in bin b, wsum[b] = sum w_i w_j.  [nb] each. */
+int gramsci_2pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
+
+/* 3pCF (S:8(a) A7, A10): every 3-clique once; counts/wsum [nb^3] at sorted triples. */
+int gramsci_3pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
+
+/* 4pCF (S:8(a) A8, A10): every 4-clique once; [nb^6] at canonical 6-tuples.
+ * Requires nbins <= 16. */
+int gramsci_4pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
+
+/* Parity-decomposed 4pCF (Eq. 3; S:8(a) A9; A-8..A-11): even == gramsci_4pcf; odd adds
+ * s = chi(raw tuple) * sign(V) per 4-clique, V from the pixel-centre unit vectors of the three spokes
+ * of the smallest-caller-label vertex, s = 0 when |V| < 1e-9 or the configuration is achiral at bin
+ * resolution.  Requires a graph built with want_pixels = 1 and nbins <= 16.  [nb^6] each. */
+int gramsci_4pcf_parity(const gramsci_graph *g, uint64_t *even_counts, int64_t *odd_counts,
+                        double *even_wsum, double *odd_wsum);
+
+/* Number of canonical configurations (3pCF: C(nb+2,3); 4pCF: S4 orbits of bin 6-tuples): 220, 680,
+ * 276, ....  Host-only arithmetic. */
+int gramsci_num_configs(int npoint /*3|4*/, int nbins, int64_t *n);
+
+/* Gather a dense HOST histogram (elem_bytes = 8) into the lexicographic list of canonical
+ * configurations: compact [n_configs] (same element type), config_bins uint8 [n_configs, 3|6].
+ * Host-only; either output may be NULL. */
+int gramsci_compact(int npoint, int nbins, const void *dense, int elem_bytes, void *compact,
+                    uint8_t *config_bins);
+
+/* Disconnected 4pCF, Eq. 4: out[c] = xi(c12)xi(c34) + xi(c13)xi(c24) + xi(c14)xi(c23) on every
+ * dense index; xi HOST [nb] -> out HOST [nb^6].  Host-only post-process (S:8(a) "tiny"). */
+int gramsci_zeta_disc(int nbins, const double *xi, double *out);
+
+/* Device time (ms, CUDA events on the graph's stream) of the kernels of the most recent call on this
+ * graph: what = 0 build (all build kernels), 1 last query total, 2 last query's enumeration kernel(s)
+ * only, 3 number of kernel launches of the last call (as a double), 4 out-of-core: bytes staged H2D. */
+int gramsci_last_timing(const gramsci_graph *g, int what, double *value);
+
+/* Exact work counters of the 3pCF on this graph (device pre-pass; S:8(d)): spoke_elems = sum over
+ * oriented edges (i,j) of len(N+(j)); tail_elems = sum of len(tail_i(j)).  HOST out-pointers. */
+int gramsci_work_counters(const gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
+
+void gramsci_free_graph(gramsci_graph *g);
+
+const char *gramsci_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAMSCI_H */

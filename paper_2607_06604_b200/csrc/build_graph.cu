@@ -1,0 +1,727 @@
+// build_graph.cu -- S:8(a) A1-A5: cell binning, neighbour count, offsets scan, fill, per-row sort.
+//
+// "finds, for each object i, all neighbors within r_max ... stored as a sorted adjacency
+// list N(i) = {j1 < j2 < ...} (Eq. 1) ... alongside each neighbor index, the radial-bin index (an
+// integer byte) and optionally a direction-pixel byte".  The paper does this on the CPU with a
+// kd-tree; here it is a GPU cell list (cells of side >= r_max, 27-cell stencil), an exclusive
+// prefix sum for the int64 row offsets ("all edge indexing is 64-bit") and, when labels are
+// not in cell order, a segmented bitonic sort of every row.
+//
+// Bit-exactness against the oracle (readings A-2..A-4, A-8): the squared distance is
+// (dx*dx + dy*dy) + dz*dz with every product and sum rounded separately (__dmul_rn/__dadd_rn are
+// never contracted into FMAs), compared with squared bin edges computed on the host.
+#include "internal.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+
+namespace {
+
+struct BuildParams {
+    int64_t n;
+    int nb;
+    int periodic;
+    double box[3], half[3];
+    double lo[3], inv_cw[3];
+    int nc[3];
+    int spatial;
+    int want_pix;
+};
+
+__constant__ double c_q[GR_MAXBINS + 1];   // squared bin edges
+__constant__ BuildParams c_bp;
+
+// ---- A1: cell ids ------------------------------------------------------------------------------
+__device__ __forceinline__ int cell_coord(double x, int c)
+{
+    int k = (int)floor((x - c_bp.lo[c]) * c_bp.inv_cw[c]);
+    k = max(0, min(k, c_bp.nc[c] - 1));
+    return k;
+}
+
+__global__ void k_cell_id(const double *__restrict__ pts, int32_t *__restrict__ cell_of,
+                          int32_t *__restrict__ cell_cnt)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c_bp.n) return;
+    int cx = cell_coord(pts[3 * i + 0], 0), cy = cell_coord(pts[3 * i + 1], 1), cz = cell_coord(pts[3 * i + 2], 2);
+    int id = (cz * c_bp.nc[1] + cy) * c_bp.nc[0] + cx;
+    cell_of[i] = id;
+    atomicAdd(&cell_cnt[id], 1);
+}
+
+__global__ void k_scatter_cells(const int32_t *__restrict__ cell_of, int32_t *__restrict__ cell_fill,
+                                int32_t *__restrict__ slot_pt, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int s = atomicAdd(&cell_fill[cell_of[i]], 1);
+    slot_pt[s] = (int32_t)i;
+}
+
+// gather coordinates (SoA) and labels into slot order
+__global__ void k_gather_slots(const double *__restrict__ pts, const int32_t *__restrict__ slot_pt,
+                               double *__restrict__ sx, double *__restrict__ sy, double *__restrict__ sz,
+                               int32_t *__restrict__ lab, int32_t *__restrict__ caller_of, int64_t n, int spatial)
+{
+    int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int32_t i = slot_pt[s];
+    sx[s] = pts[3 * (int64_t)i + 0];
+    sy[s] = pts[3 * (int64_t)i + 1];
+    sz[s] = pts[3 * (int64_t)i + 2];
+    lab[s] = spatial ? (int32_t)s : i;
+    if (caller_of) caller_of[s] = i;
+}
+
+__global__ void k_gather_weights(const double *__restrict__ w, const int32_t *__restrict__ slot_pt,
+                                 double *__restrict__ out, int64_t n, int spatial)
+{
+    int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int32_t i = slot_pt[s];
+    out[spatial ? s : (int64_t)i] = w ? w[i] : 1.0;
+}
+
+// ---- bounding box of an open catalogue ------------------------------------------------------------
+__global__ void k_minmax(const double *__restrict__ pts, int64_t n, double *__restrict__ part)
+{
+    __shared__ double s[6][256];
+    double mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        for (int c = 0; c < 3; ++c) {
+            double v = pts[3 * i + c];
+            mn[c] = fmin(mn[c], v);
+            mx[c] = fmax(mx[c], v);
+        }
+    for (int c = 0; c < 3; ++c) { s[c][threadIdx.x] = mn[c]; s[3 + c][threadIdx.x] = mx[c]; }
+    __syncthreads();
+    for (int st = 128; st > 0; st >>= 1) {
+        if ((int)threadIdx.x < st)
+            for (int c = 0; c < 3; ++c) {
+                s[c][threadIdx.x] = fmin(s[c][threadIdx.x], s[c][threadIdx.x + st]);
+                s[3 + c][threadIdx.x] = fmax(s[3 + c][threadIdx.x], s[3 + c][threadIdx.x + st]);
+            }
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) part[blockIdx.x * 6 + threadIdx.x] = s[threadIdx.x][0];
+}
+
+// ---- A3: exclusive prefix sum, int32 counts -> int64 offsets (three-phase scan) -----------------------
+constexpr int SCAN_BLOCK = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_BLOCK * SCAN_ITEMS;
+
+template <typename OutT>
+__global__ void k_scan_tile_sums(const int32_t *__restrict__ in, int64_t n, int64_t *__restrict__ tile_sum)
+{
+    __shared__ int64_t s[SCAN_BLOCK];
+    int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+    int64_t acc = 0;
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        int64_t i = base + (int64_t)k * SCAN_BLOCK + threadIdx.x;
+        if (i < n) acc += in[i];
+    }
+    s[threadIdx.x] = acc;
+    __syncthreads();
+    for (int st = SCAN_BLOCK / 2; st > 0; st >>= 1) {
+        if ((int)threadIdx.x < st) s[threadIdx.x] += s[threadIdx.x + st];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tile_sum[blockIdx.x] = s[0];
+}
+
+__global__ void k_scan_tile_offsets(int64_t *__restrict__ tile_sum, int64_t n_tiles)
+{
+    // single block: serial-in-chunks exclusive scan of the tile sums (n_tiles <= ~1e6)
+    __shared__ int64_t s[1024];
+    __shared__ int64_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < n_tiles; base += 1024) {
+        int64_t i = base + threadIdx.x;
+        int64_t v = (i < n_tiles) ? tile_sum[i] : 0;
+        s[threadIdx.x] = v;
+        __syncthreads();
+        for (int st = 1; st < 1024; st <<= 1) {
+            int64_t t = ((int)threadIdx.x >= st) ? s[threadIdx.x - st] : 0;
+            __syncthreads();
+            s[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < n_tiles) tile_sum[i] = carry + s[threadIdx.x] - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry += s[1023];
+        __syncthreads();
+    }
+}
+
+template <typename OutT>
+__global__ void k_scan_apply(const int32_t *__restrict__ in, int64_t n, const int64_t *__restrict__ tile_off,
+                             OutT *__restrict__ out)
+{
+    // each thread owns SCAN_ITEMS consecutive items
+    __shared__ int64_t s[SCAN_BLOCK];
+    int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int32_t v[SCAN_ITEMS];
+    int64_t acc = 0;
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        v[k] = (base + k < n) ? in[base + k] : 0;
+        acc += v[k];
+    }
+    s[threadIdx.x] = acc;
+    __syncthreads();
+    for (int st = 1; st < SCAN_BLOCK; st <<= 1) {
+        int64_t t = ((int)threadIdx.x >= st) ? s[threadIdx.x - st] : 0;
+        __syncthreads();
+        s[threadIdx.x] += t;
+        __syncthreads();
+    }
+    int64_t run = tile_off[blockIdx.x] + s[threadIdx.x] - acc;
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        if (base + k < n) out[base + k] = (OutT)run;
+        run += v[k];
+    }
+    if (base <= n - 1 && n - 1 < base + SCAN_ITEMS) out[n] = (OutT)run;   // total
+}
+
+template <typename OutT>
+void exclusive_scan(const int32_t *d_in, int64_t n, OutT *d_out, cudaStream_t st)
+{
+    if (n == 0) {
+        GR_CUDA(cudaMemsetAsync(d_out, 0, sizeof(OutT), st));
+        return;
+    }
+    int64_t tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
+    DevBuf<int64_t> ts;
+    ts.alloc((size_t)tiles);
+    k_scan_tile_sums<OutT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p);
+    k_scan_tile_offsets<<<1, 1024, 0, st>>>(ts.p, tiles);
+    k_scan_apply<OutT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p, d_out);
+    GR_CUDA(cudaGetLastError());
+    GR_CUDA(cudaStreamSynchronize(st));   // ts freed on return
+}
+
+// ---- A5: segmented bitonic sort (key int32 ascending, optional two byte payloads) ----------------------
+// One CTA per segment.  The network is the all-ascending form of the bitonic sorter (first step of
+// every merge stage pairs t with its mirror image, later steps pair t with t^j), so a segment whose
+// length is not a power of two is handled by treating the missing tail as +infinity: such pairs are
+// already ordered and are skipped.  Segments of at most `cap` entries are sorted in shared memory,
+// longer ones (not reached by the paper-shaped workloads) in place in global memory.
+constexpr int SORT_SMEM_CAP = 16384;
+
+__device__ __forceinline__ void bitonic_pair(int k, int j, bool first, int t, int &lo, int &hi)
+{
+    if (first) {                       // j == k/2: mirror pairing inside blocks of k
+        int base = (t / j) * k, off = t % j;
+        lo = base + off;
+        hi = base + k - 1 - off;
+    } else {
+        lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+        hi = lo | j;
+    }
+}
+
+template <typename OffT>
+__global__ void __launch_bounds__(256)
+k_segsort(const OffT *__restrict__ seg, int64_t seg_lo, int64_t seg_hi, int64_t e0, int cap,
+          int32_t *__restrict__ keys, uint8_t *__restrict__ p1, uint8_t *__restrict__ p2)
+{
+    extern __shared__ unsigned char smem_raw[];
+    int32_t *sk = (int32_t *)smem_raw;
+    uint16_t *sp = (uint16_t *)(sk + cap);
+    const int nt = blockDim.x;
+    for (int64_t r = seg_lo + blockIdx.x; r < seg_hi; r += gridDim.x) {
+        const int64_t b = (int64_t)seg[r] - e0, e = (int64_t)seg[r + 1] - e0;
+        const int len = (int)(e - b);
+        if (len < 2) continue;
+        int P = 1;
+        while (P < len) P <<= 1;
+        if (len <= cap) {
+            for (int t = threadIdx.x; t < len; t += nt) {
+                sk[t] = keys[b + t];
+                uint16_t pay = 0;
+                if (p1) pay = p1[b + t];
+                if (p2) pay |= (uint16_t)p2[b + t] << 8;
+                sp[t] = pay;
+            }
+            __syncthreads();
+            for (int k = 2; k <= P; k <<= 1)
+                for (int j = k >> 1; j > 0; j >>= 1) {
+                    for (int t = threadIdx.x; t < (P >> 1); t += nt) {
+                        int lo, hi;
+                        bitonic_pair(k, j, j == (k >> 1), t, lo, hi);
+                        if (hi < len) {
+                            int32_t a = sk[lo], c = sk[hi];
+                            if (a > c) {
+                                sk[lo] = c; sk[hi] = a;
+                                uint16_t pa = sp[lo]; sp[lo] = sp[hi]; sp[hi] = pa;
+                            }
+                        }
+                    }
+                    __syncthreads();
+                }
+            for (int t = threadIdx.x; t < len; t += nt) {
+                keys[b + t] = sk[t];
+                if (p1) p1[b + t] = (uint8_t)(sp[t] & 0xff);
+                if (p2) p2[b + t] = (uint8_t)(sp[t] >> 8);
+            }
+            __syncthreads();
+        } else {
+            for (int k = 2; k <= P; k <<= 1)
+                for (int j = k >> 1; j > 0; j >>= 1) {
+                    for (int t = threadIdx.x; t < (P >> 1); t += nt) {
+                        int lo, hi;
+                        bitonic_pair(k, j, j == (k >> 1), t, lo, hi);
+                        if (hi < len) {
+                            int32_t a = keys[b + lo], c = keys[b + hi];
+                            if (a > c) {
+                                keys[b + lo] = c; keys[b + hi] = a;
+                                if (p1) { uint8_t x = p1[b + lo]; p1[b + lo] = p1[b + hi]; p1[b + hi] = x; }
+                                if (p2) { uint8_t x = p2[b + lo]; p2[b + lo] = p2[b + hi]; p2[b + hi] = x; }
+                            }
+                        }
+                    }
+                    __syncthreads();
+                }
+        }
+    }
+}
+
+// ---- A2 / A4: neighbour count and fill ------------------------------------------------------------------
+__device__ __forceinline__ double sep1(double a, double b, int c)
+{   // separation component from a to b, minimum image when periodic (A-4)
+    double d = __dsub_rn(b, a);
+    if (c_bp.periodic) {
+        if (d > c_bp.half[c]) d = __dsub_rn(d, c_bp.box[c]);
+        else if (d < -c_bp.half[c]) d = __dadd_rn(d, c_bp.box[c]);
+    }
+    return d;
+}
+
+__device__ __forceinline__ int bin_of(double d2)
+{   // b = #{k in [1,nb): q_k <= d2} (A-3); q is non-decreasing so this is an upper bound search
+    int lo = 1, hi = c_bp.nb;            // answer = (first k in [1,nb) with q_k > d2) - 1
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (c_q[mid] <= d2) lo = mid + 1; else hi = mid;
+    }
+    return lo - 1;
+}
+
+__device__ __forceinline__ int pixel_of(double dx, double dy, double dz, double d2)
+{   // A-8: 16 equal-area z bands x 16 phi sectors
+    const double r = __dsqrt_rn(d2);
+    int iz = 0;
+#pragma unroll
+    for (int k = 1; k < 16; ++k) iz += (dz >= __dmul_rn((double)k / 8.0 - 1.0, r)) ? 1 : 0;
+    const double ax = fabs(dx), ay = fabs(dy);
+    int s = 0;
+    s += (ay >= __dmul_rn(ax, 0.41421356237309503)) ? 1 : 0;   // tan 22.5 deg
+    s += (ay >= __dmul_rn(ax, 1.0)) ? 1 : 0;                   // tan 45 deg
+    s += (ay >= __dmul_rn(ax, 2.414213562373095)) ? 1 : 0;     // tan 67.5 deg
+    int iphi;
+    if (dx >= 0.0) iphi = (dy >= 0.0) ? s : 15 - s;
+    else           iphi = (dy >= 0.0) ? 7 - s : 8 + s;
+    return 16 * iz + iphi;
+}
+
+// One warp per slot s (a point in cell order).  Lanes 0..26 own the stencil cells; duplicates (periodic
+// grids with fewer than 3 cells on an axis) are removed with match_any, and the cells are visited in
+// ascending id so that in spatial mode (label == slot) the row is emitted already sorted (Eq. 1).
+template <bool FILL>
+__global__ void __launch_bounds__(256)
+k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const double *__restrict__ sz,
+             const int32_t *__restrict__ lab, const int32_t *__restrict__ cell_start,
+             int64_t slot_lo, int64_t slot_hi, int32_t row_lo, int32_t row_hi,
+             int32_t *__restrict__ deg, const int64_t *__restrict__ ptr, int64_t e0,
+             int32_t *__restrict__ idx, uint8_t *__restrict__ bin, uint8_t *__restrict__ pix)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t s = slot_lo + ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / 32;
+    if (s >= slot_hi) return;
+    const int32_t li = lab[s];
+    if (li < row_lo || li >= row_hi) return;
+    const double xi = sx[s], yi = sy[s], zi = sz[s];
+    const int cx = cell_coord(xi, 0), cy = cell_coord(yi, 1), cz = cell_coord(zi, 2);
+    const int own = (cz * c_bp.nc[1] + cy) * c_bp.nc[0] + cx;
+
+    // stencil cell of this lane
+    int id = -1;
+    if (lane < 27) {
+        int o[3] = {cx + (lane % 3) - 1, cy + ((lane / 3) % 3) - 1, cz + (lane / 9) - 1};
+        bool ok = true;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if (c_bp.periodic) o[c] = (o[c] + c_bp.nc[c]) % c_bp.nc[c];
+            else if (o[c] < 0 || o[c] >= c_bp.nc[c]) ok = false;
+        }
+        if (ok) id = (o[2] * c_bp.nc[1] + o[1]) * c_bp.nc[0] + o[0];
+        if (c_bp.spatial && id < own) id = -1;          // label > own label  =>  cell >= own cell
+    }
+    const unsigned same = __match_any_sync(0xffffffffu, id);
+    const bool keep = (id >= 0) && ((__ffs(same) - 1) == lane);
+    int rank = 0;
+    for (int t = 0; t < 27; ++t) {
+        int v = __shfl_sync(0xffffffffu, id, t);
+        bool kt = __shfl_sync(0xffffffffu, (int)keep, t);
+        rank += (kt && v < id) ? 1 : 0;
+    }
+    const int ncell = __popc(__ballot_sync(0xffffffffu, keep));
+    int cs = 0, ce = 0;
+    if (keep) { cs = cell_start[id]; ce = cell_start[id + 1]; }
+
+    int64_t out = 0;
+    if (FILL) out = ptr[li] - e0;
+    int count = 0;
+    for (int r = 0; r < ncell; ++r) {
+        const int src = __ffs(__ballot_sync(0xffffffffu, keep && rank == r)) - 1;
+        int b = __shfl_sync(0xffffffffu, cs, src);
+        const int e = __shfl_sync(0xffffffffu, ce, src);
+        const int cid = __shfl_sync(0xffffffffu, id, src);
+        if (c_bp.spatial && cid == own) b = (int)s + 1;
+        for (int t0 = b; t0 < e; t0 += 32) {
+            const int t = t0 + lane;
+            bool edge = false;
+            int lj = 0, bb = 0, pp = 0;
+            if (t < e) {
+                lj = lab[t];
+                if (lj > li) {
+                    // direction lower label -> higher label (hub -> spoke)
+                    const double dx = sep1(xi, sx[t], 0), dy = sep1(yi, sy[t], 1), dz = sep1(zi, sz[t], 2);
+                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                    edge = (d2 >= c_q[0]) && (d2 < c_q[c_bp.nb]);      // r_min <= r < r_max (A-2)
+                    if (FILL && edge) {
+                        bb = bin_of(d2);
+                        if (c_bp.want_pix) pp = pixel_of(dx, dy, dz, d2);
+                    }
+                }
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, edge);
+            if (FILL) {
+                if (edge) {
+                    const int64_t o = out + __popc(m & ((1u << lane) - 1u));
+                    idx[o] = lj;
+                    bin[o] = (uint8_t)bb;
+                    if (pix) pix[o] = (uint8_t)pp;
+                }
+                out += __popc(m);
+            } else {
+                count += __popc(m);
+            }
+        }
+    }
+    if (!FILL && lane == 0) deg[li] = count;
+}
+
+// ---- export in caller labels (spatial mode): re-orient every edge to lower caller label ---------------
+__global__ void k_export_count(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+                               const int32_t *__restrict__ caller_of, int64_t n, int32_t *__restrict__ deg)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int ci = caller_of[i];
+    for (int64_t e = ptr[i]; e < ptr[i + 1]; ++e) {
+        int cj = caller_of[idx[e]];
+        atomicAdd(&deg[min(ci, cj)], 1);
+    }
+}
+
+__global__ void k_export_fill(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+                              const uint8_t *__restrict__ bin, const int32_t *__restrict__ caller_of, int64_t n,
+                              const int64_t *__restrict__ optr, int32_t *__restrict__ fill,
+                              int32_t *__restrict__ oidx, uint8_t *__restrict__ obin)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int ci = caller_of[i];
+    for (int64_t e = ptr[i]; e < ptr[i + 1]; ++e) {
+        int cj = caller_of[idx[e]];
+        int lo = min(ci, cj), hi = max(ci, cj);
+        int64_t o = optr[lo] + atomicAdd(&fill[lo], 1);
+        oidx[o] = hi;
+        obin[o] = bin[e];
+    }
+}
+
+inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64_t>(1, (n + per - 1) / per); }
+
+template <typename OffT>
+__global__ void k_seg_max(const OffT *__restrict__ seg, int64_t n, int32_t *__restrict__ out)
+{
+    int m = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        m = max(m, (int)(seg[i + 1] - seg[i]));
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(out, m);
+}
+
+template <typename OffT>
+int seg_max(const OffT *seg, int64_t n, cudaStream_t st)
+{
+    DevBuf<int32_t> mx;
+    mx.alloc(1);
+    int h = 0;
+    GR_CUDA(cudaMemsetAsync(mx.p, 0, sizeof(int32_t), st));
+    if (n > 0) k_seg_max<OffT><<<296, 256, 0, st>>>(seg, n, mx.p);
+    GR_CUDA(cudaMemcpyAsync(&h, mx.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    GR_CUDA(cudaStreamSynchronize(st));
+    return h;
+}
+
+// sort every segment [seg[r], seg[r+1]) for r in [seg_lo,seg_hi); max_len = longest segment
+template <typename OffT>
+void segsort(const OffT *seg, int64_t seg_lo, int64_t seg_hi, int64_t e0, int max_len, int32_t *keys, uint8_t *p1,
+             uint8_t *p2, cudaStream_t st)
+{
+    if (seg_hi <= seg_lo || max_len < 2) return;
+    int cap = 64;
+    while (cap < max_len && cap < SORT_SMEM_CAP) cap <<= 1;
+    size_t smem = (size_t)cap * (sizeof(int32_t) + sizeof(uint16_t));
+    GR_CUDA(cudaFuncSetAttribute(k_segsort<OffT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)((size_t)SORT_SMEM_CAP * 6)));
+    int threads = std::max(32, std::min(256, cap / 2));
+    unsigned grid = (unsigned)std::min<int64_t>(seg_hi - seg_lo, 148 * 32);
+    k_segsort<OffT><<<grid, threads, smem, st>>>(seg, seg_lo, seg_hi, e0, cap, keys, p1, p2);
+    GR_CUDA(cudaGetLastError());
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------
+void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced)
+{
+    const int64_t n = g->n;
+    cudaStream_t st = g->stream;
+    GrTimer timer(st);
+    double launches = 0;
+
+    // --- cell grid (cells of side >= r_max; A1) ---
+    double lo[3] = {0, 0, 0}, hi[3] = {1, 1, 1};
+    if (g->periodic) {
+        for (int c = 0; c < 3; ++c) { lo[c] = 0.0; hi[c] = g->box[c]; }
+    } else if (n > 0) {
+        const int nbk = 256;
+        DevBuf<double> part;
+        part.alloc(nbk * 6);
+        k_minmax<<<nbk, 256, 0, st>>>(d_points, n, part.p);
+        launches += 1;
+        std::vector<double> h(nbk * 6);
+        GR_CUDA(cudaMemcpyAsync(h.data(), part.p, sizeof(double) * nbk * 6, cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        for (int c = 0; c < 3; ++c) { lo[c] = INFINITY; hi[c] = -INFINITY; }
+        for (int b = 0; b < nbk; ++b)
+            for (int c = 0; c < 3; ++c) {
+                lo[c] = std::min(lo[c], h[b * 6 + c]);
+                hi[c] = std::max(hi[c], h[b * 6 + 3 + c]);
+            }
+        for (int c = 0; c < 3; ++c)
+            if (!std::isfinite(lo[c]) || !std::isfinite(hi[c])) GR_FAIL(GRAMSCI_EINVAL, "non-finite coordinate");
+    }
+    BuildParams bp;
+    bp.n = n; bp.nb = g->nb; bp.periodic = g->periodic; bp.spatial = g->spatial; bp.want_pix = g->has_pix;
+    int64_t ncell = 1;
+    // keep the cell count modest: at most ~2 cells per point and 2^22 overall
+    const double cell_budget = std::min<double>(4194304.0, std::max<double>(64.0, 2.0 * (double)n));
+    double side = g->r_max * 1.000001;
+    for (int iter = 0; iter < 64; ++iter) {
+        ncell = 1;
+        for (int c = 0; c < 3; ++c) {
+            double ext = hi[c] - lo[c];
+            int k = (ext > 0) ? (int)std::floor(ext / side) : 1;
+            k = std::max(1, std::min(k, 1024));
+            g->nc[c] = k;
+            ncell *= k;
+        }
+        if ((double)ncell <= cell_budget) break;
+        side *= 1.26;
+    }
+    for (int c = 0; c < 3; ++c) {
+        double ext = hi[c] - lo[c];
+        g->lo[c] = lo[c];
+        g->cw[c] = (ext > 0) ? ext / g->nc[c] : 1.0;
+        bp.box[c] = g->box[c]; bp.half[c] = 0.5 * g->box[c];
+        bp.lo[c] = g->lo[c]; bp.inv_cw[c] = 1.0 / g->cw[c]; bp.nc[c] = g->nc[c];
+        // guard: rounding in (x-lo)*inv_cw must not push two points closer than r_max two cells apart
+        bp.inv_cw[c] *= (1.0 - 1e-12);
+    }
+    GR_CUDA(cudaMemcpyToSymbolAsync(c_bp, &bp, sizeof(bp), 0, cudaMemcpyHostToDevice, st));
+    GR_CUDA(cudaMemcpyToSymbolAsync(c_q, g->q, sizeof(double) * (g->nb + 1), 0, cudaMemcpyHostToDevice, st));
+
+    g->ptr.alloc((size_t)n + 1);
+    g->w.alloc((size_t)n);
+    g->order.alloc((size_t)n);
+    if (g->spatial) g->caller_of.alloc((size_t)n);
+    if (n == 0) {
+        GR_CUDA(cudaMemsetAsync(g->ptr.p, 0, sizeof(int64_t), st));
+        g->idx.alloc(0); g->bin.alloc(0);
+        if (g->has_pix) g->pix.alloc(0);
+        g->windows.clear();
+        GrWindow w0; g->windows.push_back(w0);
+        g->n_edges = 0; g->max_row = 0;
+        GR_CUDA(cudaStreamSynchronize(st));
+        g->t_build_ms = timer.stop();
+        g->n_launches = launches;
+        return;
+    }
+
+    // --- counting sort of the points by cell, ascending caller index inside a cell (A1) ---
+    DevBuf<int32_t> cell_of, cell_cnt, cell_start, cell_fill, slot_pt;
+    cell_of.alloc((size_t)n);
+    cell_cnt.alloc((size_t)ncell);
+    cell_start.alloc((size_t)ncell + 1);
+    cell_fill.alloc((size_t)ncell + 1);
+    slot_pt.alloc((size_t)n);
+    GR_CUDA(cudaMemsetAsync(cell_cnt.p, 0, sizeof(int32_t) * ncell, st));
+    k_cell_id<<<blocks_for(n, 256), 256, 0, st>>>(d_points, cell_of.p, cell_cnt.p);
+    exclusive_scan<int32_t>(cell_cnt.p, ncell, cell_start.p, st);
+    GR_CUDA(cudaMemcpyAsync(cell_fill.p, cell_start.p, sizeof(int32_t) * (ncell + 1), cudaMemcpyDeviceToDevice, st));
+    k_scatter_cells<<<blocks_for(n, 256), 256, 0, st>>>(cell_of.p, cell_fill.p, slot_pt.p, n);
+    segsort<int32_t>(cell_start.p, 0, ncell, 0, seg_max<int32_t>(cell_start.p, ncell, st), slot_pt.p, nullptr, nullptr, st);
+    launches += 6;
+
+    DevBuf<double> sx, sy, sz;
+    DevBuf<int32_t> lab;
+    sx.alloc((size_t)n); sy.alloc((size_t)n); sz.alloc((size_t)n); lab.alloc((size_t)n);
+    k_gather_slots<<<blocks_for(n, 256), 256, 0, st>>>(d_points, slot_pt.p, sx.p, sy.p, sz.p, lab.p,
+                                                       g->spatial ? g->caller_of.p : nullptr, n, g->spatial);
+    k_gather_weights<<<blocks_for(n, 256), 256, 0, st>>>(d_weights, slot_pt.p, g->w.p, n, g->spatial);
+    GR_CUDA(cudaMemcpyAsync(g->order.p, lab.p, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, st));
+    launches += 2;
+
+    // --- A2 count, A3 offsets ---
+    DevBuf<int32_t> deg;
+    deg.alloc((size_t)n);
+    const unsigned nblk = blocks_for(n * 32, 256);
+    k_neighbours<false><<<nblk, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, deg.p,
+                                              nullptr, 0, nullptr, nullptr, nullptr);
+    exclusive_scan<int64_t>(deg.p, n, g->ptr.p, st);
+    launches += 4;
+    int64_t E = 0;
+    GR_CUDA(cudaMemcpyAsync(&E, g->ptr.p + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    GR_CUDA(cudaStreamSynchronize(st));
+    g->max_row = seg_max<int64_t>(g->ptr.p, n, st);
+    launches += 1;
+    g->n_edges = E;
+
+    // --- windows (row-aligned): one window in-core, several when a memory cap is set ---
+    const uint64_t bpe = 5 + (g->has_pix ? 1 : 0);
+    std::vector<int64_t> hptr;
+    g->windows.clear();
+    int W = 1;
+    g->ooc = 0;
+    if (g->cap_bytes && ((uint64_t)E * bpe > g->cap_bytes || n_windows_forced > 1)) {
+        g->ooc = 1;
+        // four window buffers must fit under the cap (hub + search, double buffered)
+        uint64_t per = g->cap_bytes / 4;
+        W = (int)(((uint64_t)E * bpe + per - 1) / std::max<uint64_t>(per, 1));
+        W = std::max(W, 2);
+    }
+    if (n_windows_forced > 0) { W = n_windows_forced; g->ooc = (g->cap_bytes != 0); }
+    if (W > 1 || g->ooc) {
+        hptr.resize((size_t)n + 1);
+        GR_CUDA(cudaMemcpyAsync(hptr.data(), g->ptr.p, sizeof(int64_t) * (n + 1), cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+    }
+    if (W <= 1) {
+        GrWindow w0;
+        w0.row_lo = 0; w0.row_hi = (int32_t)n; w0.e_lo = 0; w0.e_hi = E;
+        g->windows.push_back(w0);
+    } else {
+        int64_t target = (E + W - 1) / W;
+        int32_t r = 0;
+        while (r < n) {
+            GrWindow w;
+            w.row_lo = r;
+            int64_t want = hptr[r] + target;
+            int32_t r2 = (int32_t)(std::upper_bound(hptr.begin() + r, hptr.end(), want) - hptr.begin()) - 1;
+            r2 = std::max(r2, r + 1);
+            r2 = (int32_t)std::min<int64_t>(r2, n);
+            w.row_hi = r2;
+            w.e_lo = hptr[r] & ~int64_t(15);
+            w.e_hi = hptr[r2];
+            g->windows.push_back(w);
+            r = r2;
+        }
+    }
+
+    // --- A4 fill (+ A5 sort when labels are not in cell order) per window ---
+    if (!g->ooc) {
+        g->idx.alloc((size_t)E);
+        g->bin.alloc((size_t)E);
+        if (g->has_pix) g->pix.alloc((size_t)E);
+        k_neighbours<true><<<nblk, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, nullptr,
+                                                 g->ptr.p, 0, g->idx.p, g->bin.p, g->has_pix ? g->pix.p : nullptr);
+        launches += 1;
+        if (!g->spatial) {
+            segsort<int64_t>(g->ptr.p, 0, n, 0, g->max_row, g->idx.p, g->bin.p, g->has_pix ? g->pix.p : nullptr, st);
+            launches += 1;
+        }
+        GR_CUDA(cudaGetLastError());
+    } else {
+        GR_CUDA(cudaHostAlloc((void **)&g->h_idx, std::max<size_t>((size_t)E * 4 + 256, 256), cudaHostAllocDefault));
+        GR_CUDA(cudaHostAlloc((void **)&g->h_bin, std::max<size_t>((size_t)E + 256, 256), cudaHostAllocDefault));
+        if (g->has_pix)
+            GR_CUDA(cudaHostAlloc((void **)&g->h_pix, std::max<size_t>((size_t)E + 256, 256), cudaHostAllocDefault));
+        int64_t maxlen = 0;
+        for (auto &w : g->windows) maxlen = std::max(maxlen, w.e_hi - w.e_lo);
+        DevBuf<int32_t> widx;
+        DevBuf<uint8_t> wbin, wpix;
+        widx.alloc((size_t)maxlen); wbin.alloc((size_t)maxlen);
+        if (g->has_pix) wpix.alloc((size_t)maxlen);
+        for (auto &w : g->windows) {
+            int64_t len = w.e_hi - w.e_lo;
+            int64_t s_lo = g->spatial ? w.row_lo : 0, s_hi = g->spatial ? w.row_hi : n;
+            unsigned nb2 = blocks_for((s_hi - s_lo) * 32, 256);
+            k_neighbours<true><<<nb2, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, s_lo, s_hi, w.row_lo, w.row_hi,
+                                                    nullptr, g->ptr.p, w.e_lo, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr);
+            launches += 1;
+            if (!g->spatial) {
+                segsort<int64_t>(g->ptr.p, w.row_lo, w.row_hi, w.e_lo, g->max_row, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr, st);
+                launches += 1;
+            }
+            int64_t head = hptr[w.row_lo] - w.e_lo;   // entries before the first row belong to the previous window
+            GR_CUDA(cudaMemcpyAsync(g->h_idx + w.e_lo + head, widx.p + head, (size_t)(len - head) * 4, cudaMemcpyDeviceToHost, st));
+            GR_CUDA(cudaMemcpyAsync(g->h_bin + w.e_lo + head, wbin.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));
+            if (g->has_pix)
+                GR_CUDA(cudaMemcpyAsync(g->h_pix + w.e_lo + head, wpix.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));
+            GR_CUDA(cudaStreamSynchronize(st));
+        }
+    }
+    GR_CUDA(cudaStreamSynchronize(st));
+    g->t_build_ms = timer.stop();
+    g->n_launches = launches;
+}
+
+// ---------------------------------------------------------------------------------------------------
+void gr_export_csr(const gramsci_graph *g, int64_t *d_ptr, int32_t *d_idx, uint8_t *d_bin, uint8_t *d_pix)
+{
+    cudaStream_t st = g->stream;
+    const int64_t n = g->n, E = g->n_edges;
+    if (g->ooc) GR_FAIL(GRAMSCI_EINVAL, "export_csr: not supported for out-of-core graphs");
+    if (!g->spatial) {
+        if (d_ptr) GR_CUDA(cudaMemcpyAsync(d_ptr, g->ptr.p, sizeof(int64_t) * (n + 1), cudaMemcpyDeviceToDevice, st));
+        if (d_idx && E) GR_CUDA(cudaMemcpyAsync(d_idx, g->idx.p, sizeof(int32_t) * E, cudaMemcpyDeviceToDevice, st));
+        if (d_bin && E) GR_CUDA(cudaMemcpyAsync(d_bin, g->bin.p, E, cudaMemcpyDeviceToDevice, st));
+        if (d_pix && E && g->has_pix) GR_CUDA(cudaMemcpyAsync(d_pix, g->pix.p, E, cudaMemcpyDeviceToDevice, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        return;
+    }
+    DevBuf<int32_t> deg, fill, oidx;
+    DevBuf<int64_t> optr;
+    DevBuf<uint8_t> obin;
+    deg.alloc((size_t)n); fill.alloc((size_t)n); optr.alloc((size_t)n + 1); oidx.alloc((size_t)E); obin.alloc((size_t)E);
+    GR_CUDA(cudaMemsetAsync(deg.p, 0, sizeof(int32_t) * std::max<int64_t>(n, 1), st));
+    GR_CUDA(cudaMemsetAsync(fill.p, 0, sizeof(int32_t) * std::max<int64_t>(n, 1), st));
+    if (n) k_export_count<<<blocks_for(n, 256), 256, 0, st>>>(g->ptr.p, g->idx.p, g->caller_of.p, n, deg.p);
+    exclusive_scan<int64_t>(deg.p, n, optr.p, st);
+    if (n) {
+        k_export_fill<<<blocks_for(n, 256), 256, 0, st>>>(g->ptr.p, g->idx.p, g->bin.p, g->caller_of.p, n, optr.p, fill.p,
+                                                          oidx.p, obin.p);
+        segsort<int64_t>(optr.p, 0, n, 0, seg_max<int64_t>(optr.p, n, st), oidx.p, obin.p, nullptr, st);
+    }
+    GR_CUDA(cudaGetLastError());
+    if (d_ptr) GR_CUDA(cudaMemcpyAsync(d_ptr, optr.p, sizeof(int64_t) * (n + 1), cudaMemcpyDeviceToDevice, st));
+    if (d_idx && E) GR_CUDA(cudaMemcpyAsync(d_idx, oidx.p, sizeof(int32_t) * E, cudaMemcpyDeviceToDevice, st));
+    if (d_bin && E) GR_CUDA(cudaMemcpyAsync(d_bin, obin.p, E, cudaMemcpyDeviceToDevice, st));
+    GR_CUDA(cudaStreamSynchronize(st));
+}

@@ -1,0 +1,150 @@
+// internal.cuh -- shared declarations of the CUDA path (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include <vector>
+
+#include "../../include/gramsci.h"
+
+#define GR_MAXBINS 255
+#define GR_SM_COUNT_FALLBACK 148
+
+// ---- error plumbing --------------------------------------------------------------------------
+void gr_set_error(const char *fmt, ...);
+struct GrFail { int code; };   // thrown inside the library only; every ABI entry catches it
+
+#define GR_CUDA(call)                                                                         \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess) {                                                              \
+            gr_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            throw GrFail{e_ == cudaErrorMemoryAllocation ? GRAMSCI_ENOMEM : GRAMSCI_ECUDA};   \
+        }                                                                                     \
+    } while (0)
+
+#define GR_FAIL(code_, ...)            \
+    do {                               \
+        gr_set_error(__VA_ARGS__);     \
+        throw GrFail{code_};           \
+    } while (0)
+
+// ---- device buffer owned by the library --------------------------------------------------------
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    DevBuf() {}
+    DevBuf(const DevBuf &) = delete;
+    DevBuf &operator=(const DevBuf &) = delete;
+    ~DevBuf() { release(); }
+    void alloc(size_t count) {
+        release();
+        n = count;
+        size_t bytes = (count ? count : 1) * sizeof(T);
+        bytes = (bytes + 255) & ~size_t(255);          // tail padding: aligned vector loads may over-read
+        GR_CUDA(cudaMalloc((void **)&p, bytes + 256));
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+};
+
+// One contiguous range of CSR rows whose edge arrays sit in one buffer (device or pinned host).
+struct GrWindow {
+    int32_t row_lo = 0, row_hi = 0;   // rows [row_lo,row_hi)
+    int64_t e_lo = 0, e_hi = 0;       // edges [e_lo,e_hi), e_lo rounded down to a multiple of 16
+};
+
+struct gramsci_graph {
+    // parameters
+    int64_t n = 0;
+    int nb = 1;
+    int periodic = 0;
+    double box[3] = {0, 0, 0};
+    double r_min = 0, r_max = 0;
+    double q[GR_MAXBINS + 1];      // squared bin edges (A-3)
+    int weighted = 0, has_pix = 0, spatial = 0, algo = 0;
+    cudaStream_t stream = nullptr;
+    int sm_count = GR_SM_COUNT_FALLBACK;
+    size_t smem_optin = 0;
+    // cell grid
+    int nc[3] = {1, 1, 1};
+    double lo[3] = {0, 0, 0}, cw[3] = {1, 1, 1};
+    // graph (internal labels; `order` lists labels in spatial order = hub schedule)
+    int64_t n_edges = 0;
+    int32_t max_row = 0;
+    DevBuf<int64_t> ptr;           // [n+1]
+    DevBuf<int32_t> idx;           // [E]   (in-core only)
+    DevBuf<uint8_t> bin, pix;      // [E]
+    DevBuf<double> w;              // [n] weights by internal label
+    DevBuf<int32_t> order;         // [n] label at spatial slot s
+    DevBuf<int32_t> caller_of;     // [n] caller label of internal label (spatial mode), else empty
+    // out-of-core state: edge arrays in pinned host memory, cut into row-aligned windows
+    uint64_t cap_bytes = 0;
+    int ooc = 0;
+    std::vector<GrWindow> windows;
+    std::vector<uint8_t> need;     // [W*W] need[h*W+c] = 1 iff some edge (i,j) has i in window h, j in window c
+    int32_t *h_idx = nullptr;      // pinned [E]
+    uint8_t *h_bin = nullptr, *h_pix = nullptr;
+    // timing of the last calls
+    double t_build_ms = 0, t_query_ms = 0, t_enum_ms = 0, n_launches = 0, staged_bytes = 0;
+};
+
+// ---- build_graph.cu -----------------------------------------------------------------------------
+void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced);
+void gr_export_csr(const gramsci_graph *g, int64_t *d_ptr, int32_t *d_idx, uint8_t *d_bin, uint8_t *d_pix);
+
+// ---- query kernels ----------------------------------------------------------------------------
+// Device views handed to the enumeration kernels: hub rows come from (idx_h,bin_h,pix_h) holding
+// edges [e0_h, ...), spoke rows from (idx_c,...) holding edges [e0_c, ...); only spokes with label
+// in [c_lo,c_hi) are processed (the out-of-core tile rule).
+struct GrView {
+    const int64_t *ptr;
+    const int32_t *idx_h; const uint8_t *bin_h; const uint8_t *pix_h; int64_t e0_h;
+    const int32_t *idx_c; const uint8_t *bin_c; const uint8_t *pix_c; int64_t e0_c;
+    int32_t h_lo, h_hi;     // hub rows of this tile (labels)
+    int32_t c_lo, c_hi;     // resident search rows (labels)
+    const int32_t *order;   // hub schedule (labels in spatial order), [n]
+    int32_t s_lo, s_hi;     // schedule slots to walk (in-core: [0,n))
+    const double *w;        // weights by label or nullptr
+};
+
+void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
+void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
+void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c, double *d_even_w, double *d_odd_w);
+void gr_work_counters(gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
+
+// tiler.cu: run `tile_fn(view)` over every needed (hub window, search window) tile
+struct GrTileRunner;
+typedef void (*gr_tile_fn)(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st);
+// hub_only: visit each hub window once with no search window (2pCF sweep, work counters)
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user);
+
+// host helpers (canon.cpp part of api.cu)
+int gr_canon4(int nb, const int t[6], int c[6]);   // returns chirality factor
+int64_t gr_num_configs4(int nb);
+
+struct GrTimer {
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaStream_t st;
+    explicit GrTimer(cudaStream_t s) : st(s) {
+        cudaEventCreate(&a);
+        cudaEventCreate(&b);
+        cudaEventRecord(a, st);
+    }
+    double stop() {
+        cudaEventRecord(b, st);
+        cudaEventSynchronize(b);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        return ms;
+    }
+    ~GrTimer() {
+        if (a) cudaEventDestroy(a);
+        if (b) cudaEventDestroy(b);
+    }
+};

@@ -1,0 +1,133 @@
+// tiler.cu -- S:8(a) A11: out-of-core window tiling.
+//
+// the edge arrays are cut into W row-aligned windows; a tile is a (hub window h, search
+// window c) pair; the tuple rooted at edge (i,j) is processed in the one tile with i in h and j in c,
+// and spokes whose row is not resident are skipped with one integer compare.  Here the windows live
+// in pinned host memory and are streamed through a small cache of device buffers on a copy stream,
+// so that the upload of the next tile's windows overlaps the enumeration of the current tile.
+// Tiles whose search window holds no spoke of the hub window (known from the build) are not visited:
+// with labels in cell order a hub window only reaches a few search windows.
+#include "internal.cuh"
+
+#include <algorithm>
+
+namespace {
+
+struct Slot {
+    DevBuf<int32_t> idx;
+    DevBuf<uint8_t> bin, pix;
+    int wid = -1;
+    cudaEvent_t ready = nullptr, done = nullptr;
+    uint64_t stamp = 0;
+};
+
+}  // namespace
+
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user)
+{
+    cudaStream_t st = g->stream;
+    GrView v;
+    v.ptr = g->ptr.p;
+    v.order = g->order.p;
+    v.w = g->w.p;
+    if (!g->ooc) {
+        v.idx_h = v.idx_c = g->idx.p;
+        v.bin_h = v.bin_c = g->bin.p;
+        v.pix_h = v.pix_c = g->has_pix ? g->pix.p : nullptr;
+        v.e0_h = v.e0_c = 0;
+        v.h_lo = v.c_lo = 0;
+        v.h_hi = v.c_hi = (int32_t)g->n;
+        v.s_lo = 0;
+        v.s_hi = (int32_t)g->n;
+        fn(g, v, user, st);
+        return;
+    }
+
+    const int W = (int)g->windows.size();
+    const uint64_t bpe = 5 + (g->has_pix ? 1 : 0);
+    int64_t maxlen = 0;
+    for (auto &w : g->windows) maxlen = std::max(maxlen, w.e_hi - w.e_lo);
+    int K = (int)std::min<uint64_t>((uint64_t)W, g->cap_bytes / std::max<uint64_t>(1, (uint64_t)maxlen * bpe));
+    K = std::min(K, 8);
+    if (K < (hub_only ? 1 : 2)) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for two windows of %lld edges", (long long)maxlen);
+
+    std::vector<Slot> slots(K);
+    cudaStream_t cs = nullptr;
+    GR_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    struct Cleanup {
+        std::vector<Slot> &s; cudaStream_t cs;
+        ~Cleanup() {
+            cudaStreamSynchronize(cs);
+            for (auto &x : s) { if (x.ready) cudaEventDestroy(x.ready); if (x.done) cudaEventDestroy(x.done); }
+            cudaStreamDestroy(cs);
+        }
+    } cleanup{slots, cs};
+    for (auto &s : slots) {
+        s.idx.alloc((size_t)maxlen + 64);
+        s.bin.alloc((size_t)maxlen + 64);
+        if (g->has_pix && need_pix) s.pix.alloc((size_t)maxlen + 64);
+        GR_CUDA(cudaEventCreateWithFlags(&s.ready, cudaEventDisableTiming));
+        GR_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+    }
+    // the copy stream must not start before earlier work on the compute stream (e.g. memsets) is ordered
+    uint64_t clock = 0;
+
+    // bring window `wid` into a slot (cache hit: no copy); never evicts a slot whose bit is set in `protect`
+    auto acquire = [&](int wid, unsigned protect) -> int {
+        for (int k = 0; k < K; ++k)
+            if (slots[k].wid == wid) { slots[k].stamp = ++clock; return k; }
+        int victim = -1;
+        for (int k = 0; k < K; ++k) {
+            if (protect & (1u << k)) continue;
+            if (victim < 0 || slots[k].stamp < slots[victim].stamp) victim = k;
+        }
+        if (victim < 0) return -1;
+        Slot &s = slots[victim];
+        const GrWindow &w = g->windows[wid];
+        const int64_t len = w.e_hi - w.e_lo;
+        if (s.wid >= 0) GR_CUDA(cudaStreamWaitEvent(cs, s.done, 0));     // last kernel reading it has finished
+        if (len > 0) {
+            GR_CUDA(cudaMemcpyAsync(s.idx.p, g->h_idx + w.e_lo, (size_t)len * 4, cudaMemcpyHostToDevice, cs));
+            GR_CUDA(cudaMemcpyAsync(s.bin.p, g->h_bin + w.e_lo, (size_t)len, cudaMemcpyHostToDevice, cs));
+            if (g->has_pix && need_pix)
+                GR_CUDA(cudaMemcpyAsync(s.pix.p, g->h_pix + w.e_lo, (size_t)len, cudaMemcpyHostToDevice, cs));
+            g->staged_bytes += (double)len * (5 + ((g->has_pix && need_pix) ? 1 : 0));
+        }
+        GR_CUDA(cudaEventRecord(s.ready, cs));
+        s.wid = wid;
+        s.stamp = ++clock;
+        return victim;
+    };
+
+    std::vector<std::pair<int, int>> tiles;
+    for (int h = 0; h < W; ++h) {
+        if (hub_only) { tiles.push_back({h, h}); continue; }
+        for (int c = 0; c < W; ++c)
+            if (g->need.empty() || g->need[(size_t)h * W + c]) tiles.push_back({h, c});
+    }
+    const int T = (int)tiles.size();
+    for (int t = 0; t < T; ++t) {
+        const int a = acquire(tiles[t].first, 0);
+        const int b = acquire(tiles[t].second, 1u << a);
+        if (a < 0 || b < 0) GR_FAIL(GRAMSCI_ENOMEM, "window cache exhausted");
+        GR_CUDA(cudaStreamWaitEvent(st, slots[a].ready, 0));
+        GR_CUDA(cudaStreamWaitEvent(st, slots[b].ready, 0));
+        const GrWindow &wh = g->windows[tiles[t].first], &wc = g->windows[tiles[t].second];
+        v.idx_h = slots[a].idx.p; v.bin_h = slots[a].bin.p; v.pix_h = slots[a].pix.p; v.e0_h = wh.e_lo;
+        v.idx_c = slots[b].idx.p; v.bin_c = slots[b].bin.p; v.pix_c = slots[b].pix.p; v.e0_c = wc.e_lo;
+        v.h_lo = wh.row_lo; v.h_hi = wh.row_hi;
+        v.c_lo = wc.row_lo; v.c_hi = wc.row_hi;
+        if (g->spatial) { v.s_lo = wh.row_lo; v.s_hi = wh.row_hi; }
+        else { v.s_lo = 0; v.s_hi = (int32_t)g->n; }
+        fn(g, v, user, st);
+        GR_CUDA(cudaEventRecord(slots[a].done, st));
+        if (b != a) GR_CUDA(cudaEventRecord(slots[b].done, st));
+        // prefetch the next tile's windows into slots the running tile does not use (copy stream)
+        if (t + 1 < T) {
+            unsigned protect = (1u << a) | (1u << b);
+            int s1 = acquire(tiles[t + 1].first, protect);
+            if (s1 >= 0) acquire(tiles[t + 1].second, protect | (1u << s1));
+        }
+    }
+    GR_CUDA(cudaStreamSynchronize(st));
+}

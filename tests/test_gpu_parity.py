@@ -1,0 +1,130 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Integer counts bit-exact; fp64 weighted sums within 1e-10 relative
+(BASELINE.json north_star; per-bin scale = sum of |prod w|, S:8(c) A-13)."""
+import numpy as np
+import pytest
+
+import catalogues as cat
+import oracle
+import paper_2607_06604_b200 as gr
+
+pytestmark = pytest.mark.gpu
+
+RTOL_W = 1e-10
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+def build_both(cfg, device_inputs=True, **opts):
+    torch = _torch()
+    pts, w, box = cfg["points"], cfg["weights"], cfg["box"]
+    og = oracle.Graph(pts, w, box, cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    if device_inputs:
+        dp = torch.from_numpy(pts).cuda()
+        dw = None if w is None else torch.from_numpy(w).cuda()
+    else:
+        dp, dw = pts, w
+    gg = gr.gramsci_build_graph(dp, dw, box, cfg["r_min"], cfg["r_max"], cfg["nbins"], **opts)
+    return og, gg
+
+
+def small(seed, n=1500, L=30.0, r_min=0.0, r_max=5.0, nb=6, weighted=False, periodic=True, snap=False):
+    pts = cat.uniform_box(n, L, seed)
+    if snap:
+        pts = cat.snap(pts)
+    w = np.random.default_rng(seed + 77).uniform(0.5, 1.5, n) if weighted else None
+    return dict(points=pts, weights=w, box=[L, L, L] if periodic else None, r_min=r_min, r_max=r_max, nbins=nb)
+
+
+def assert_weighted_close(got, want, scale=None):
+    scale = np.abs(want) if scale is None else scale
+    assert np.all(np.abs(got - want) <= RTOL_W * np.maximum(scale, 1e-300) + 0.0), \
+        float(np.max(np.abs(got - want) / np.maximum(scale, 1e-300)))
+
+
+@pytest.mark.parametrize("relabel", [1, 2])
+@pytest.mark.parametrize("periodic,r_min,snap", [(True, 0.0, False), (False, 0.0, False), (True, 1.7, True)])
+def test_graph_matches_oracle(relabel, periodic, r_min, snap):
+    cfg = small(11, periodic=periodic, r_min=r_min, snap=snap)
+    og, gg = build_both(cfg, relabel=relabel, want_pixels=(relabel == 2))
+    o_ptr, o_idx, o_bin, o_pix = og.csr()
+    if relabel == 2:
+        ptr, idx, b, p = gg.export_csr(want_pix=True)
+        assert np.array_equal(p, o_pix)
+    else:
+        ptr, idx, b = gg.export_csr()
+    assert np.array_equal(ptr, o_ptr)
+    assert np.array_equal(idx, o_idx)
+    assert np.array_equal(b, o_bin)
+    assert gg.info()["n_edges"] == og.n_edges
+
+
+@pytest.mark.parametrize("relabel", [1, 2])
+def test_2pcf(relabel):
+    cfg = small(12, weighted=True)
+    og, gg = build_both(cfg, relabel=relabel)
+    oc, ow = og.pcf2()
+    c, w = gg.pcf2(weighted=True)
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+
+
+@pytest.mark.parametrize("algo", [gr.ALGO_BSEARCH])
+@pytest.mark.parametrize("relabel", [1, 2])
+def test_3pcf_config1(relabel, algo):
+    cfg = cat.config1()
+    og, gg = build_both(cfg, relabel=relabel, algo=algo)
+    oc, _ = og.pcf3()
+    c, _ = gg.pcf3()
+    assert c.sum() == oc.sum()
+    assert np.array_equal(c, oc)
+    # host-buffer path gives the same
+    c2, _ = gg.pcf3(host=True)
+    assert np.array_equal(c2, oc)
+
+
+@pytest.mark.parametrize("algo", [gr.ALGO_BSEARCH])
+@pytest.mark.parametrize("periodic,r_min", [(True, 0.0), (False, 0.0), (True, 2.0)])
+def test_3pcf_weighted(periodic, r_min, algo):
+    cfg = small(13, n=4000, L=40.0, weighted=True, periodic=periodic, r_min=r_min, nb=7)
+    og, gg = build_both(cfg, device_inputs=False, algo=algo)
+    oc, ow = og.pcf3()
+    c, w = gg.pcf3(weighted=True)
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+
+
+def test_edge_cases():
+    torch = _torch()
+    # empty catalogue, single point, no edges, one triangle
+    for pts in (np.zeros((0, 3)), np.array([[0.5, 0.5, 0.5]]), np.array([[0.1, 0.1, 0.1], [5.0, 5.0, 5.0]])):
+        g = gr.gramsci_build_graph(pts, None, [10.0, 10.0, 10.0], 0.0, 1.0, 3)
+        assert g.info()["n_edges"] == 0
+        c, _ = g.pcf3(host=True)
+        assert c.sum() == 0
+        c2, _ = g.pcf2(host=True)
+        assert c2.sum() == 0
+    tri = np.array([[1.0, 1.0, 1.0], [1.5, 1.0, 1.0], [1.0, 1.9, 1.0]])
+    g = gr.gramsci_build_graph(tri, None, None, 0.0, 3.0, 3)
+    og = oracle.Graph(tri, None, None, 0.0, 3.0, 3)
+    c, _ = g.pcf3(host=True)
+    assert np.array_equal(c, og.pcf3()[0]) and c.sum() == 1
+    # coincident points are an edge iff r_min == 0 (A-6)
+    dup = np.array([[1.0, 1.0, 1.0], [1.0, 1.0, 1.0], [1.2, 1.0, 1.0]])
+    for r_min in (0.0, 0.1):
+        g = gr.gramsci_build_graph(dup, None, None, r_min, 1.0, 2)
+        og = oracle.Graph(dup, None, None, r_min, 1.0, 2)
+        assert g.info()["n_edges"] == og.n_edges
+        assert np.array_equal(g.pcf3(host=True)[0], og.pcf3()[0])
+    # periodic box with fewer than three cells per axis (stencil aliasing)
+    cfg = small(14, n=600, L=10.0, r_max=4.5, nb=4)
+    og, gg = build_both(cfg)
+    assert np.array_equal(gg.pcf3()[0], og.pcf3()[0])
+    # errors
+    with pytest.raises(gr.GramsciError) as e:
+        gr.gramsci_build_graph(cfg["points"], None, [10.0, 10.0, 10.0], 0.0, 5.0, 4)
+    assert e.value.code == 2
