@@ -21,7 +21,7 @@ import numpy as np
 __all__ = [
     "uniform_box", "neyman_scott", "survey_wedge", "snap",
     "config1", "config2_data", "config2_randoms", "config3", "config4", "config5",
-    "isolated_units", "CONFIGS",
+    "isolated_units", "tetra_from_lengths", "SCALENE_EDGES", "CONFIGS",
 ]
 
 
@@ -123,6 +123,20 @@ def config5(seed: int = 5001, n: int = 2_500_000, L: float = 1700.0):
     """configs[4]: BAO-scale 3pCF, 2.5e6 uniform points, periodic L=1700, 60<=r<150, 18 bins.
     The scaled replica cfg5' uses L=425, n=39_062 (same density)."""
     return _cfg(uniform_box(n, L, seed), None, [L, L, L], 60.0, 150.0, 18, "3pcf", "cfg5")
+
+
+SCALENE_EDGES = (4.5, 5.5, 6.5, 7.5, 8.5, 9.5)   # l01 < l02 < l03 < l12 < l13 < l23
+
+
+def tetra_from_lengths(l01, l02, l03, l12, l13, l23) -> np.ndarray:
+    """Vertex coordinates [4,3] of a tetrahedron with the given edge lengths (v3 on the +z side)."""
+    x2 = (l01 ** 2 + l02 ** 2 - l12 ** 2) / (2 * l01)
+    y2 = float(np.sqrt(l02 ** 2 - x2 ** 2))
+    x3 = (l01 ** 2 + l03 ** 2 - l13 ** 2) / (2 * l01)
+    y3 = (l02 ** 2 + l03 ** 2 - l23 ** 2 - 2 * x2 * x3) / (2 * y2)
+    z3sq = l03 ** 2 - x3 ** 2 - y3 ** 2
+    assert z3sq > 0.5, "tetrahedron not embeddable / too flat"
+    return np.array([[0.0, 0.0, 0.0], [l01, 0.0, 0.0], [x2, y2, 0.0], [x3, y3, float(np.sqrt(z3sq))]])
 
 
 def _random_rotations(k: int, rng) -> np.ndarray:

@@ -1,6 +1,342 @@
-// query4.cu -- placeholder until the 4pCF kernels land (S:8(a) A8, A9).
+// query4.cu -- S:8(a) A8 (4pCF second-level intersection), A9 (parity split), A10 (fold + flush).
+//
+// tetrahedra are the tuples (i, j1, j2, j3) whose six pairs are all graph edges; P:72-87 finds j3
+// by walking three sorted lists at once, P:149 instead precomputes, per hub, the "local connectivity
+// matrix lmat(k2,k1)" holding the bin of the edge between two hub neighbours, so that the innermost
+// loop is O(1) lookups after C(m,2) membership searches per hub.  This file takes the second design
+// and restates it for a CTA:
+//
+//   phase 1 (per hub i, = the 3pCF membership pass): row a of the local matrix D is
+//            D[a][p] = bin of edge (k_a, k_p) if k_p in N+(k_a) else 0xFF,   a < p < n = len(N+(i)),
+//            found by one lane-parallel search of every element of N+(k_a) in the staged hub row;
+//   phase 2: for every local edge (a,b) (D[a][b] != 0xFF) a warp streams rows a and b of D with
+//            coalesced 4-byte loads; every c > b with D[a][c] and D[b][c] both set is a 4-clique
+//            i < k_a < k_b < k_c, found exactly once (oriented storage, A-1, A-15), and is histogrammed by
+//            its raw 6-tuple (b_ia, b_ib, b_ic, b_ab, b_ac, b_bc) = the order (b12,b13,b14,b23,b24,b34).
+//
+// Parity (Eq. 3; A-8..A-11): V = (n_a x n_b) . n_c on the pixel-centre unit vectors of the three
+// hub spokes, every product and sum rounded separately; the kernel accumulates sign(V) (0 when
+// |V| < 1e-9) per RAW tuple and the fold applies the chirality factor of the raw tuple, which for the
+// raw tuple t^sigma of a canonical chiral tuple t is sgn(sigma) (and 0 for bin-achiral t).
+//
+// D lives in a per-CTA slice of a global scratch (the paper's "per-gang slice of a global scratch sized
+// from the longest row"); it is written and read by the same CTA only and stays in L1/L2.
+// Raw histograms are nb^6 bins -- too large for shared memory (8^6 x 4 B = 1 MiB) -- so hits go to
+// global memory with RED atomics, spread over a few shards that the fold sums.
 #include "internal.cuh"
-void gr_4pcf(gramsci_graph *, int, uint64_t *, int64_t *, double *, double *)
+
+#include <algorithm>
+#include <cmath>
+
+namespace {
+
+constexpr int Q4_THREADS = 256;
+constexpr int Q4_WARPS = Q4_THREADS / 32;
+
+struct Q4Params {
+    int nb;
+    int64_t nh;          // nb^6
+    int row_cap;         // staged hub row capacity (multiple of 16)
+    int parity, weighted, want_counts;
+    int n_shards;
+};
+
+__constant__ int8_t c_perm4[24][4] = {
+    {0,1,2,3},{0,1,3,2},{0,2,1,3},{0,2,3,1},{0,3,1,2},{0,3,2,1},{1,0,2,3},{1,0,3,2},{1,2,0,3},{1,2,3,0},
+    {1,3,0,2},{1,3,2,0},{2,0,1,3},{2,0,3,1},{2,1,0,3},{2,1,3,0},{2,3,0,1},{2,3,1,0},{3,0,1,2},{3,0,2,1},
+    {3,1,0,2},{3,1,2,0},{3,2,0,1},{3,2,1,0}};
+
+__device__ __forceinline__ int lower_bound_s(const int32_t *a, int lo, int hi, int32_t key)
 {
-    GR_FAIL(GRAMSCI_EINVAL, "4pcf: not implemented yet");
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        if (a[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// ---- enumeration ---------------------------------------------------------------------------------------
+// cnt_e/cnt_o/w_e/w_o: [n_shards][nh] raw histograms (any may be null).
+__global__ void __launch_bounds__(Q4_THREADS)
+k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *scratch, size_t scratch_stride,
+       const double *__restrict__ pix_tab, unsigned long long *__restrict__ cnt_e,
+       unsigned long long *__restrict__ cnt_o, double *__restrict__ w_e, double *__restrict__ w_o)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    // layout: [tab 256*3*8 (parity)] [w row_cap*8 (weighted)] [idx row_cap*4] [t3 row_cap*4] [pix row_cap]
+    double *s_tab = (double *)smem;
+    double *a_w = (double *)(smem + (p.parity ? 256 * 3 * 8 : 0));
+    int32_t *a_idx = (int32_t *)((unsigned char *)a_w + (p.weighted ? (size_t)p.row_cap * 8 : 0));
+    uint32_t *a_t3 = (uint32_t *)(a_idx + p.row_cap);       // b_ic * nb^3
+    uint8_t *a_pix = (uint8_t *)(a_t3 + p.row_cap);
+    __shared__ int s_slot;
+
+    const int nb = p.nb;
+    const uint32_t nb2 = nb * nb, nb3 = nb2 * nb;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint8_t *D = scratch + (size_t)blockIdx.x * scratch_stride;
+    const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh;
+    if (cnt_e) cnt_e += shard;
+    if (cnt_o) cnt_o += shard;
+    if (w_e) w_e += shard;
+    if (w_o) w_o += shard;
+    if (p.parity)
+        for (int t = threadIdx.x; t < 256 * 3; t += Q4_THREADS) s_tab[t] = pix_tab[t];
+
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_slot = v.s_lo + (int)atomicAdd(hub_counter, 1u);
+        __syncthreads();
+        const int s = s_slot;
+        if (s >= v.s_hi) break;
+        const int32_t i = v.order[s];
+        const int64_t rb = v.ptr[i], re = v.ptr[i + 1];
+        const int n = (int)(re - rb);
+        if (n < 3) continue;                                   // a 4-clique needs three spokes
+        const int ld = (n + 15) & ~15;                         // row stride of D
+        const int32_t *gi = v.idx_h + (rb - v.e0_h);
+        const uint8_t *gb = v.bin_h + (rb - v.e0_h);
+        const uint8_t *gp = v.pix_h ? v.pix_h + (rb - v.e0_h) : nullptr;
+        for (int t = threadIdx.x; t < n; t += Q4_THREADS) {
+            const int32_t k = gi[t];
+            a_idx[t] = k;
+            a_t3[t] = (uint32_t)gb[t] * nb3;
+            if (p.parity) a_pix[t] = gp[t];
+            if (p.weighted) a_w[t] = v.w[k];
+        }
+        // D := 0xFF
+        {
+            uint4 ff = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+            uint4 *D4 = (uint4 *)D;
+            const int total = (n * ld) >> 4;
+            for (int t = threadIdx.x; t < total; t += Q4_THREADS) D4[t] = ff;
+        }
+        __syncthreads();
+
+        // ---- phase 1: local connectivity matrix ----
+        for (int a = warp; a < n - 1; a += Q4_WARPS) {
+            const int32_t j = a_idx[a];
+            const int64_t jb = v.ptr[j], je = v.ptr[j + 1];
+            const int nj = (int)(je - jb);
+            const int32_t *B = v.idx_c + (jb - v.e0_c);
+            const uint8_t *Bb = v.bin_c + (jb - v.e0_c);
+            const int32_t t_last = a_idx[n - 1];
+            uint8_t *Da = D + (size_t)a * ld;
+            int lo = a + 1;
+            for (int t0 = 0; t0 < nj; t0 += 32) {
+                const int t = t0 + lane;
+                const int32_t k = (t < nj) ? B[t] : INT32_MAX;
+                int pos = n;
+                if (k <= t_last) pos = lower_bound_s(a_idx, lo, n, k);
+                if (pos < n && a_idx[pos] == k) Da[pos] = Bb[t];
+                lo = __shfl_sync(0xffffffffu, pos, 0);
+                if (__shfl_sync(0xffffffffu, k, 31) > t_last) break;
+            }
+        }
+        __syncthreads();
+
+        // ---- phase 2: triangles of the local graph = 4-cliques under hub i ----
+        const double wi = p.weighted ? v.w[i] : 1.0;
+        for (int a = 0; a < n - 2; ++a) {
+            const uint8_t *Da = D + (size_t)a * ld;
+            const uint32_t base_a = (a_t3[a] / nb3) * (nb3 * nb2);             // b_ia * nb^5
+            double na0 = 0, na1 = 0, na2 = 0;
+            if (p.parity) { const double *q = s_tab + 3 * a_pix[a]; na0 = q[0]; na1 = q[1]; na2 = q[2]; }
+            const double wia = p.weighted ? wi * a_w[a] : 1.0;
+            for (int b = a + 1 + warp; b < n - 1; b += Q4_WARPS) {
+                const uint32_t g_ab = Da[b];
+                if (g_ab == 0xffu) continue;
+                const uint8_t *Db = D + (size_t)b * ld;
+                const uint32_t base = base_a + (a_t3[b] / nb3) * (nb3 * nb) + g_ab * nb2;   // + b_ib nb^4 + b_ab nb^2
+                double cx = 0, cy = 0, cz = 0;
+                if (p.parity) {
+                    const double *q = s_tab + 3 * a_pix[b];
+                    const double nb0 = q[0], nb1 = q[1], nb2d = q[2];
+                    cx = __dsub_rn(__dmul_rn(na1, nb2d), __dmul_rn(na2, nb1));
+                    cy = __dsub_rn(__dmul_rn(na2, nb0), __dmul_rn(na0, nb2d));
+                    cz = __dsub_rn(__dmul_rn(na0, nb1), __dmul_rn(na1, nb0));
+                }
+                const double wiab = p.weighted ? wia * a_w[b] : 1.0;
+                for (int c0 = ((b + 1) & ~3) + 4 * lane; c0 < n; c0 += 128) {
+                    const uint32_t ra = *(const uint32_t *)(Da + c0);
+                    const uint32_t rbw = *(const uint32_t *)(Db + c0);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int c = c0 + q;
+                        const uint32_t g_ac = (ra >> (8 * q)) & 0xffu, g_bc = (rbw >> (8 * q)) & 0xffu;
+                        if (c > b && c < n && g_ac != 0xffu && g_bc != 0xffu) {
+                            const uint32_t x = base + a_t3[c] + g_ac * nb + g_bc;
+                            if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
+                            double ww = 0.0;
+                            if (p.weighted) {
+                                ww = wiab * a_w[c];
+                                atomicAdd(&w_e[x], ww);
+                            }
+                            if (p.parity) {
+                                const double *nc = s_tab + 3 * a_pix[c];
+                                const double V = __dadd_rn(__dadd_rn(__dmul_rn(cx, nc[0]), __dmul_rn(cy, nc[1])),
+                                                           __dmul_rn(cz, nc[2]));
+                                if (fabs(V) >= 1e-9) {
+                                    const bool pos = V > 0.0;
+                                    if (cnt_o) atomicAdd(&cnt_o[x], pos ? 1ull : ~0ull);     // += +-1 (mod 2^64)
+                                    if (w_o) atomicAdd(&w_o[x], pos ? ww : -ww);
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ---- A10 fold: raw 6-tuples -> canonical configurations (A-7), odd channel with the chirality sign (A-10) ---
+__global__ void k_fold4(int nb, int64_t nh, int n_shards, const unsigned long long *__restrict__ cnt_e,
+                        const unsigned long long *__restrict__ cnt_o, const double *__restrict__ w_e,
+                        const double *__restrict__ w_o, unsigned long long *__restrict__ out_ce,
+                        long long *__restrict__ out_co, double *__restrict__ out_we, double *__restrict__ out_wo)
+{
+    const int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= nh) return;
+    int t[6];
+    {
+        int64_t r = x;
+        for (int e = 5; e >= 0; --e) { t[e] = (int)(r % nb); r /= nb; }
+    }
+    int m[4][4];
+    m[0][0] = m[1][1] = m[2][2] = m[3][3] = 0;
+    m[0][1] = m[1][0] = t[0]; m[0][2] = m[2][0] = t[1]; m[0][3] = m[3][0] = t[2];
+    m[1][2] = m[2][1] = t[3]; m[1][3] = m[3][1] = t[4]; m[2][3] = m[3][2] = t[5];
+    int64_t ys[24];
+    bool canonical = true, odd_aut = false;
+    for (int s = 0; s < 24; ++s) {
+        const int8_t *q = c_perm4[s];
+        const int u[6] = {m[q[0]][q[1]], m[q[0]][q[2]], m[q[0]][q[3]], m[q[1]][q[2]], m[q[1]][q[3]], m[q[2]][q[3]]};
+        int64_t y = 0;
+        for (int e = 0; e < 6; ++e) y = y * nb + u[e];
+        ys[s] = y;
+        if (y < x) canonical = false;            // base-nb value order == lexicographic order of the tuple
+        int inv = 0;
+        for (int a = 0; a < 4; ++a)
+            for (int b = a + 1; b < 4; ++b) inv += (q[a] > q[b]) ? 1 : 0;
+        if (y == x && (inv & 1)) odd_aut = true; // an odd vertex order fixes the tuple: achiral at bin resolution
+    }
+    unsigned long long ce = 0;
+    long long co = 0;
+    double we = 0.0, wo = 0.0;
+    if (canonical) {
+        for (int s = 0; s < 24; ++s) {
+            bool dup = false;
+            for (int r = 0; r < s; ++r) dup = dup || (ys[r] == ys[s]);
+            if (dup) continue;
+            const int8_t *q = c_perm4[s];
+            int inv = 0;
+            for (int a = 0; a < 4; ++a)
+                for (int b = a + 1; b < 4; ++b) inv += (q[a] > q[b]) ? 1 : 0;
+            const int sg = (inv & 1) ? -1 : 1;
+            for (int sh = 0; sh < n_shards; ++sh) {
+                const size_t y = (size_t)sh * (size_t)nh + (size_t)ys[s];
+                if (cnt_e) ce += cnt_e[y];
+                if (w_e) we += w_e[y];
+                if (!odd_aut) {
+                    if (cnt_o) co += (long long)sg * (long long)cnt_o[y];
+                    if (w_o) wo += (double)sg * w_o[y];
+                }
+            }
+        }
+    }
+    if (out_ce) out_ce[x] = ce;
+    if (out_co) out_co[x] = co;
+    if (out_we) out_we[x] = we;
+    if (out_wo) out_wo[x] = wo;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------
+void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c, double *d_even_w, double *d_odd_w)
+{
+    cudaStream_t st = g->stream;
+    const int nb = g->nb;
+    if (g->ooc) GR_FAIL(GRAMSCI_EINVAL, "4pcf: out-of-core graphs are not supported (build without device_mem_cap_bytes)");
+    int64_t nh = 1;
+    for (int e = 0; e < 6; ++e) nh *= nb;
+    GrTimer total(st);
+    g->n_launches = 0;
+    g->staged_bytes = 0;
+
+    Q4Params p;
+    p.nb = nb; p.nh = nh;
+    p.parity = parity ? 1 : 0;
+    p.weighted = (d_even_w || d_odd_w) ? 1 : 0;
+    p.want_counts = (d_even_c || d_odd_c) ? 1 : 0;
+    p.row_cap = std::max(16, (g->max_row + 15) & ~15);
+    const int channels = (d_even_c ? 1 : 0) + (d_odd_c ? 1 : 0) + (d_even_w ? 1 : 0) + (d_odd_w ? 1 : 0);
+    if (channels == 0) { GR_CUDA(cudaStreamSynchronize(st)); g->t_query_ms = total.stop(); return; }
+    p.n_shards = (int)std::max<int64_t>(1, std::min<int64_t>(8, ((int64_t)64 << 20) / (nh * 8 * channels)));
+
+    size_t smem = (p.parity ? 256 * 3 * 8 : 0) + (size_t)p.row_cap * (4 + 4 + 1 + (p.weighted ? 8 : 0)) + 64;
+    if (smem > g->smem_optin)
+        GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
+    GR_CUDA(cudaFuncSetAttribute(k_4pcf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_4pcf, Q4_THREADS, smem));
+    occ = std::max(1, std::min(occ, 4));
+    const int grid = g->sm_count * occ;
+    const size_t stride = (size_t)p.row_cap * p.row_cap;
+
+    DevBuf<uint8_t> scratch;
+    DevBuf<unsigned int> counter;
+    DevBuf<double> tab;
+    DevBuf<unsigned long long> ce, co;
+    DevBuf<double> we, wo;
+    scratch.alloc(stride * grid);
+    counter.alloc(1);
+    GR_CUDA(cudaMemsetAsync(counter.p, 0, sizeof(unsigned int), st));
+    const size_t tot = (size_t)nh * p.n_shards;
+    if (d_even_c) { ce.alloc(tot); GR_CUDA(cudaMemsetAsync(ce.p, 0, tot * 8, st)); }
+    if (d_odd_c) { co.alloc(tot); GR_CUDA(cudaMemsetAsync(co.p, 0, tot * 8, st)); }
+    if (d_even_w || d_odd_w) { we.alloc(tot); GR_CUDA(cudaMemsetAsync(we.p, 0, tot * 8, st)); }
+    if (d_odd_w) { wo.alloc(tot); GR_CUDA(cudaMemsetAsync(wo.p, 0, tot * 8, st)); }
+    if (p.parity) {
+        // pixel-centre unit vectors (A-8): z_c = (iz + 1/2)/8 - 1, phi_c = (iphi + 1/2) pi/8
+        std::vector<double> h(256 * 3);
+        for (int px = 0; px < 256; ++px) {
+            const int iz = px >> 4, ip = px & 15;
+            const double zc = ((double)iz + 0.5) / 8.0 - 1.0;
+            const double ph = ((double)ip + 0.5) * (3.14159265358979323846 / 8.0);
+            const double sq = std::sqrt(1.0 - zc * zc);
+            h[3 * px + 0] = sq * std::cos(ph);
+            h[3 * px + 1] = sq * std::sin(ph);
+            h[3 * px + 2] = zc;
+        }
+        tab.alloc(256 * 3);
+        GR_CUDA(cudaMemcpyAsync(tab.p, h.data(), sizeof(double) * 256 * 3, cudaMemcpyHostToDevice, st));
+        GR_CUDA(cudaStreamSynchronize(st));      // h goes out of scope
+    }
+
+    GrView v;
+    v.ptr = g->ptr.p; v.order = g->order.p; v.w = g->w.p;
+    v.idx_h = v.idx_c = g->idx.p; v.bin_h = v.bin_c = g->bin.p;
+    v.pix_h = v.pix_c = g->has_pix ? g->pix.p : nullptr;
+    v.e0_h = v.e0_c = 0;
+    v.h_lo = v.c_lo = 0; v.h_hi = v.c_hi = (int32_t)g->n;
+    v.s_lo = 0; v.s_hi = (int32_t)g->n;
+    {
+        GrTimer en(st);
+        if (g->n > 0) {
+            k_4pcf<<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
+                                                   (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
+            GR_CUDA(cudaGetLastError());
+            g->n_launches += 1;
+        }
+        g->t_enum_ms = en.stop();
+    }
+    k_fold4<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, p.n_shards, ce.p, co.p, d_even_w ? we.p : nullptr, wo.p,
+                                                          (unsigned long long *)d_even_c, (long long *)d_odd_c,
+                                                          d_even_w, d_odd_w);
+    GR_CUDA(cudaGetLastError());
+    g->n_launches += 1;
+    GR_CUDA(cudaStreamSynchronize(st));
+    g->t_query_ms = total.stop();
 }

@@ -128,3 +128,86 @@ def test_edge_cases():
     with pytest.raises(gr.GramsciError) as e:
         gr.gramsci_build_graph(cfg["points"], None, [10.0, 10.0, 10.0], 0.0, 5.0, 4)
     assert e.value.code == 2
+
+
+# ---- 4pCF and parity-decomposed 4pCF (S:8(a) A8-A10) --------------------------------------------------
+@pytest.mark.parametrize("relabel", [1, 2])
+@pytest.mark.parametrize("periodic,r_min,nb", [(True, 0.0, 4), (False, 0.0, 6), (True, 1.5, 3)])
+def test_4pcf(relabel, periodic, r_min, nb):
+    cfg = small(21, n=3000, L=30.0, weighted=True, periodic=periodic, r_min=r_min, r_max=5.0, nb=nb)
+    og, gg = build_both(cfg, relabel=relabel)
+    oc, ow = og.pcf4()
+    assert oc.sum() > 1000
+    c, w = gg.pcf4(weighted=True)
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+    # counts only, straight into host memory
+    c2, _ = gg.pcf4(host=True)
+    assert np.array_equal(c2, oc)
+    # the disconnected term needs the 2pCF of the same graph (Eq. 4, A-12)
+    assert np.array_equal(gg.pcf2()[0], og.pcf2()[0])
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+def test_4pcf_parity(periodic):
+    cfg = small(22, n=3000, L=30.0, weighted=True, periodic=periodic, r_max=5.0, nb=5)
+    og, gg = build_both(cfg, want_pixels=True)
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    assert np.abs(oc).sum() > 100
+    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
+    assert np.array_equal(gec, ec)
+    assert np.array_equal(goc, oc)
+    assert_weighted_close(gew, ew)
+    assert_weighted_close(gow, ow, scale=np.abs(ew))      # A-13: scale = sum |prod w| of the bin
+    # even channel == plain 4pCF; parity needs pixels and caller labels
+    assert np.array_equal(gg.pcf4()[0], ec)
+    _, g2 = build_both(cfg)
+    with pytest.raises(gr.GramsciError) as e:
+        g2.pcf4_parity()
+    assert e.value.code == 1
+
+
+def test_4pcf_parity_wedge():
+    """Scaled replica of BASELINE configs[3] (survey wedge, open box, weights U(0.8,1.2), 8 bins)."""
+    cfg = cat.config4(seed=4002, n=6000, cap_deg=7.0)
+    og, gg = build_both(cfg, want_pixels=True)
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    assert ec.sum() > 10000
+    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
+    assert np.array_equal(gec, ec)
+    assert np.array_equal(goc, oc)
+    assert_weighted_close(gew, ew)
+    assert_weighted_close(gow, ow, scale=np.abs(ew))
+
+
+def test_4pcf_injection_on_gpu():
+    """P:261 injection idea on the CUDA path: isolated scalene tetrahedra, mirrored fraction 30 %."""
+    r_min, r_max, nb = 4.0, 10.0, 6
+    tet = cat.tetra_from_lengths(*cat.SCALENE_EDGES)
+    K = 200
+    mirror = np.zeros(K, dtype=bool)
+    mirror[: int(0.3 * K)] = True
+    pts, _, _ = cat.isolated_units(tet, K, spacing=40.0, seed=91, mirror_mask=mirror)
+    og = oracle.Graph(pts, None, None, r_min, r_max, nb)
+    gg = gr.gramsci_build_graph(pts, None, None, r_min, r_max, nb, want_pixels=True)
+    ec, _, oc, _ = og.pcf4(parity=True)
+    gec, goc, _, _ = gg.pcf4_parity()
+    i6 = np.ravel_multi_index((0, 1, 2, 3, 4, 5), (nb,) * 6)
+    assert gec[i6] == K and gec.sum() == K
+    assert np.array_equal(gec, ec) and np.array_equal(goc, oc)
+    assert abs(goc[i6] - (K - 2 * int(mirror.sum()))) <= 0.04 * K
+
+
+def test_4pcf_edge_cases():
+    _torch()
+    for pts in (np.zeros((0, 3)), np.array([[0.5, 0.5, 0.5]]), np.array([[1.0, 1.0, 1.0], [1.5, 1.0, 1.0], [1.0, 1.9, 1.0]])):
+        g = gr.gramsci_build_graph(pts, None, None, 0.0, 3.0, 2, want_pixels=True)
+        ec, oc, _, _ = g.pcf4_parity(host=True)
+        assert ec.sum() == 0 and not oc.any()
+    # one regular tetrahedron -> one 4-clique in bin (0,0,0,0,0,0)
+    tet = np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], dtype=np.float64) * 0.3 + 5.0
+    g = gr.gramsci_build_graph(tet, None, None, 0.0, 3.0, 3)
+    c, _ = g.pcf4(host=True)
+    assert c.sum() == 1 and c[0] == 1
+    with pytest.raises(gr.GramsciError):
+        gr.gramsci_build_graph(tet, None, None, 0.0, 3.0, 17).pcf4()
