@@ -57,7 +57,12 @@ enum {
     GRAMSCI_ALGO_DEFAULT = 0,
     GRAMSCI_ALGO_MERGEPATH = 1, /* merge-path partitioned two-list intersection (P:57-70 on a warp) */
     GRAMSCI_ALGO_BSEARCH = 2,   /* lane-parallel binary search of N+(j) in the hub tail */
-    GRAMSCI_ALGO_BITMAP = 3     /* hub row scattered into a shared-memory slot table, O(1) membership */
+    GRAMSCI_ALGO_BITMAP = 3,    /* hub row scattered into a shared-memory slot table, O(1) membership;
+                                   the default when the table fits (labels in cell order)               */
+    GRAMSCI_ALGO_TABLE_G1 = 4,  /* slot table with a forced number of warps per hub: 1, 2, 4, 8          */
+    GRAMSCI_ALGO_TABLE_G2 = 5,
+    GRAMSCI_ALGO_TABLE_G4 = 6,
+    GRAMSCI_ALGO_TABLE_G8 = 7
 };
 
 typedef struct {       /* zero-initialised struct == defaults */

@@ -28,6 +28,7 @@ ABI_SYMBOLS = [
 ]
 
 ALGO_DEFAULT, ALGO_MERGEPATH, ALGO_BSEARCH, ALGO_BITMAP = 0, 1, 2, 3
+ALGO_TABLE_G1, ALGO_TABLE_G2, ALGO_TABLE_G4, ALGO_TABLE_G8 = 4, 5, 6, 7
 
 STATUS = {0: "GRAMSCI_OK", 1: "GRAMSCI_EINVAL", 2: "GRAMSCI_ERANGE", 3: "GRAMSCI_ENOMEM", 4: "GRAMSCI_ECUDA",
           5: "GRAMSCI_EOVERFLOW"}

@@ -106,7 +106,7 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     gramsci_options o;
     memset(&o, 0, sizeof o);
     if (opt) o = *opt;
-    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 3 || o.n_windows < 0)
+    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0)
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: bad options");
     require_device();
 

@@ -443,6 +443,53 @@ __global__ void k_export_fill(const int64_t *__restrict__ ptr, const int32_t *__
     }
 }
 
+// ---- row statistics for the slot-table 3pCF kernel: one warp per row -------------------------------------
+// out[0] = max over rows of (last - first); out[1 + s - GR_S_MIN] = max over rows of the number of
+// distinct pages ((k - first) >> s) among the row's entries.  Rows are sorted, so a page starts where
+// an entry's page differs from its predecessor's.
+__global__ void __launch_bounds__(256)
+k_row_stats(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, int64_t e0, int32_t row_lo,
+            int32_t row_hi, int32_t *__restrict__ out)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t r = row_lo + ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / 32;
+    if (r >= row_hi) return;
+    const int64_t b = ptr[r] - e0, e = ptr[r + 1] - e0;
+    if (e - b < 1) return;
+    const int32_t first = idx[b], last = idx[e - 1];
+    int cnt[GR_S_MAX - GR_S_MIN + 1];
+#pragma unroll
+    for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) cnt[s] = 0;
+    int32_t carry = -1;                        // d of the previous chunk's last entry
+    for (int64_t t0 = b; t0 < e; t0 += 32) {
+        const int64_t t = t0 + lane;
+        const int32_t d = (t < e) ? idx[t] - first : 0;
+        int32_t prev = __shfl_up_sync(0xffffffffu, d, 1);
+        if (lane == 0) prev = carry;
+#pragma unroll
+        for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) {
+            const bool np = (t < e) && (prev < 0 || (d >> (s + GR_S_MIN)) != (prev >> (s + GR_S_MIN)));
+            cnt[s] += __popc(__ballot_sync(0xffffffffu, np));
+        }
+        carry = __shfl_sync(0xffffffffu, d, 31);
+    }
+    if (lane == 0) {
+        atomicMax(&out[0], last - first);
+#pragma unroll
+        for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) atomicMax(&out[1 + s], cnt[s]);
+    }
+}
+
+// largest neighbour label stored in edges [lo,hi) (which search windows a hub window reaches; tiler.cu)
+__global__ void k_max_label(const int32_t *__restrict__ idx, int64_t lo, int64_t hi, int32_t *__restrict__ out)
+{
+    int m = -1;
+    for (int64_t e = lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < hi; e += (int64_t)gridDim.x * blockDim.x)
+        m = max(m, idx[e]);
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m >= 0) atomicMax(out, m);
+}
+
 inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64_t>(1, (n + per - 1) / per); }
 
 template <typename OffT>
@@ -627,15 +674,19 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         w0.row_lo = 0; w0.row_hi = (int32_t)n; w0.e_lo = 0; w0.e_hi = E;
         g->windows.push_back(w0);
     } else {
-        int64_t target = (E + W - 1) / W;
+        // boundaries at the first row starting at or after k*E/W (k = 1..W-1); empty windows are dropped
         int32_t r = 0;
-        while (r < n) {
+        for (int k = 1; k <= W && r < n; ++k) {
+            int32_t r2 = (int32_t)n;
+            if (k < W) {
+                const int64_t want = (int64_t)(((__int128)E * k) / W);
+                r2 = (int32_t)(std::lower_bound(hptr.begin(), hptr.begin() + n, want) - hptr.begin());
+                r2 = std::max(r2, r + 1);
+                r2 = (int32_t)std::min<int64_t>(r2, n);
+                if (hptr[r2] == hptr[r] && r2 < n) continue;      // no edges yet: extend this window
+            }
             GrWindow w;
             w.row_lo = r;
-            int64_t want = hptr[r] + target;
-            int32_t r2 = (int32_t)(std::upper_bound(hptr.begin() + r, hptr.end(), want) - hptr.begin()) - 1;
-            r2 = std::max(r2, r + 1);
-            r2 = (int32_t)std::min<int64_t>(r2, n);
             w.row_hi = r2;
             w.e_lo = hptr[r] & ~int64_t(15);
             w.e_hi = hptr[r2];
@@ -643,6 +694,10 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             r = r2;
         }
     }
+
+    DevBuf<int32_t> stats;
+    stats.alloc(16);
+    GR_CUDA(cudaMemsetAsync(stats.p, 0, sizeof(int32_t) * 16, st));
 
     // --- A4 fill (+ A5 sort when labels are not in cell order) per window ---
     if (!g->ooc) {
@@ -656,6 +711,8 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             segsort<int64_t>(g->ptr.p, 0, n, 0, g->max_row, g->idx.p, g->bin.p, g->has_pix ? g->pix.p : nullptr, st);
             launches += 1;
         }
+        k_row_stats<<<blocks_for(n * 32, 256), 256, 0, st>>>(g->ptr.p, g->idx.p, 0, 0, (int32_t)n, stats.p);
+        launches += 1;
         GR_CUDA(cudaGetLastError());
     } else {
         GR_CUDA(cudaHostAlloc((void **)&g->h_idx, std::max<size_t>((size_t)E * 4 + 256, 256), cudaHostAllocDefault));
@@ -668,6 +725,11 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         DevBuf<uint8_t> wbin, wpix;
         widx.alloc((size_t)maxlen); wbin.alloc((size_t)maxlen);
         if (g->has_pix) wpix.alloc((size_t)maxlen);
+        const int Wn = (int)g->windows.size();
+        g->need.assign((size_t)Wn * Wn, 0);
+        DevBuf<int32_t> dmax;
+        dmax.alloc(1);
+        int hwin = 0;
         for (auto &w : g->windows) {
             int64_t len = w.e_hi - w.e_lo;
             int64_t s_lo = g->spatial ? w.row_lo : 0, s_hi = g->spatial ? w.row_hi : n;
@@ -679,7 +741,20 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
                 segsort<int64_t>(g->ptr.p, w.row_lo, w.row_hi, w.e_lo, g->max_row, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr, st);
                 launches += 1;
             }
+            k_row_stats<<<blocks_for((int64_t)(w.row_hi - w.row_lo) * 32, 256), 256, 0, st>>>(g->ptr.p, widx.p, w.e_lo,
+                                                                                           w.row_lo, w.row_hi, stats.p);
+            launches += 1;
             int64_t head = hptr[w.row_lo] - w.e_lo;   // entries before the first row belong to the previous window
+            // search windows this hub window reaches: spokes have larger labels than their hub, so [hwin, window of the largest label]
+            int32_t hmax = -1;
+            GR_CUDA(cudaMemsetAsync(dmax.p, 0xff, sizeof(int32_t), st));
+            if (len > head) k_max_label<<<296, 256, 0, st>>>(widx.p, head, len, dmax.p);
+            GR_CUDA(cudaMemcpyAsync(&hmax, dmax.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+            GR_CUDA(cudaStreamSynchronize(st));
+            launches += 1;
+            for (int c = hwin; c < Wn; ++c)
+                if (hmax >= g->windows[c].row_lo) g->need[(size_t)hwin * Wn + c] = 1;
+            ++hwin;
             GR_CUDA(cudaMemcpyAsync(g->h_idx + w.e_lo + head, widx.p + head, (size_t)(len - head) * 4, cudaMemcpyDeviceToHost, st));
             GR_CUDA(cudaMemcpyAsync(g->h_bin + w.e_lo + head, wbin.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));
             if (g->has_pix)
@@ -687,7 +762,13 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             GR_CUDA(cudaStreamSynchronize(st));
         }
     }
-    GR_CUDA(cudaStreamSynchronize(st));
+    {
+        int32_t h[16];
+        GR_CUDA(cudaMemcpyAsync(h, stats.p, sizeof h, cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        g->max_span = h[0];
+        for (int s = GR_S_MIN; s <= GR_S_MAX; ++s) g->max_pages[s] = h[1 + s - GR_S_MIN];
+    }
     g->t_build_ms = timer.stop();
     g->n_launches = launches;
 }

@@ -10,6 +10,8 @@
 
 #define GR_MAXBINS 255
 #define GR_SM_COUNT_FALLBACK 148
+#define GR_S_MIN 3
+#define GR_S_MAX 12
 
 // ---- error plumbing --------------------------------------------------------------------------
 void gr_set_error(const char *fmt, ...);
@@ -83,6 +85,10 @@ struct gramsci_graph {
     DevBuf<double> w;              // [n] weights by internal label
     DevBuf<int32_t> order;         // [n] label at spatial slot s
     DevBuf<int32_t> caller_of;     // [n] caller label of internal label (spatial mode), else empty
+    // row statistics for the slot-table 3pCF kernel (query3.cu): label span of a row (last - first) and,
+    // for page size 2^s labels (s = GR_S_MIN .. GR_S_MAX), the number of distinct pages a row touches
+    int32_t max_span = 0;
+    int32_t max_pages[16] = {0};
     // out-of-core state: edge arrays in pinned host memory, cut into row-aligned windows
     uint64_t cap_bytes = 0;
     int ooc = 0;

@@ -14,6 +14,8 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
+#include <type_traits>
 
 namespace {
 
@@ -147,6 +149,252 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
     }
 }
 
+// ---- 3pCF, slot-table variant (default) ------------------------------------------------------------------
+// Membership of k in N+(i) is one table lookup instead of a search (the hub-side analogue of the paper's
+// lmat idea: spend O(len) setup per hub to make every later test O(1)).  The hub row is scattered
+// into a two-level table keyed by d = k - first(N+(i)):  page g = d >> s  ->  chunk pt[g] (0 = page not
+// touched by the row), slot (chunk << s) | (d & (2^s - 1)) -> the entry's bin byte (or its position,
+// weighted) or EMPTY.  With labels in cell order a row touches few pages (it lives in a handful of runs
+// of x-adjacent cells), so the table is a few KB; sizes come from the row statistics of the build.
+// Set-up and tear-down touch only the row's own entries (O(len)).
+//
+// Work mapping: G warps share one hub (G = 1, 2, 4, 8 by table size); each warp takes blocks of 32 spokes
+// and walks the concatenation of their rows N+(j) as ONE flat index space ("every lane always has an
+// element": rows are tens of entries long in the 1e6-point configurations, so a per-row 32-lane loop would
+// idle a third of the lanes and serialise the ptr -> idx load latency per row).  The spoke a lane's element
+// belongs to is recovered from a start-bit mask of the rows beginning inside the 32-element window.
+template <int G>
+__device__ __forceinline__ void group_sync(int group)
+{
+    if (G == 1) __syncwarp();
+    else if (G == Q3_WARPS) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(G * 32) : "memory");
+}
+
+struct T3Params {
+    int nb, nh;
+    int s;              // page shift
+    int pt_len;         // page-table entries (uint16)
+    int tab_len;        // slots
+    int row_cap;        // staged weights / bins per hub (weighted)
+    int want_counts;
+    int group_bytes;    // shared memory per group (multiple of 16)
+    int hub_batch;      // schedule slots fetched per atomic
+};
+
+template <bool WEIGHTED, int G>
+__global__ void __launch_bounds__(Q3_THREADS)
+k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
+             unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
+{
+    typedef typename std::conditional<WEIGHTED, uint16_t, uint8_t>::type slot_t;
+    constexpr unsigned EMPTY = WEIGHTED ? 0xffffu : 0xffu;
+    constexpr int NGROUPS = Q3_WARPS / G;
+    extern __shared__ __align__(16) unsigned char smem[];
+    // CTA: [hist u32 nh] [group 0] [group 1] ...
+    uint32_t *hist = (uint32_t *)smem;
+    double *my_w = WEIGHTED ? g_w + (size_t)blockIdx.x * p.nh : nullptr;   // fp64 partials: one slab per CTA (RED.F64)
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    const int group = warp / G, gw = warp % G;
+    // (plain pointer arithmetic on `smem` only: a round trip through an integer would turn every access
+    // below into a generic-address load instead of LDS)
+    unsigned char *gs = smem + (((size_t)p.nh * 4 + 15) & ~(size_t)15) + (size_t)group * p.group_bytes;
+    // group: [a_w f64 row_cap (W)] [flat arrays per warp] [pt u16] [tab] [a_bin u8 row_cap (W)]
+    double *a_w = (double *)gs;
+    unsigned char *q = gs + (WEIGHTED ? (size_t)p.row_cap * 8 : 0);
+    long long *s_base = (long long *)q + gw * 32;           q += (size_t)G * 32 * 8;
+    double *s_wia = (double *)q + gw * 32;                  q += WEIGHTED ? (size_t)G * 32 * 8 : 0;
+    int *s_hb = (int *)q + gw * 32;                         q += (size_t)G * 32 * 4;
+    int *s_off = (int *)q + gw * 32;                        q += (size_t)G * 32 * 4;
+    uint16_t *pt = (uint16_t *)q;                           q += ((size_t)p.pt_len * 2 + 15) & ~(size_t)15;
+    slot_t *tab = (slot_t *)q;                              q += ((size_t)p.tab_len * sizeof(slot_t) + 15) & ~(size_t)15;
+    uint8_t *a_bin = (uint8_t *)q;
+    __shared__ int s_fetch[NGROUPS];
+
+    for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) hist[t] = 0;
+    for (int t = gw * 32 + lane; t < p.pt_len; t += G * 32) pt[t] = 0;
+    for (int t = gw * 32 + lane; t < p.tab_len; t += G * 32) tab[t] = (slot_t)EMPTY;
+    __syncthreads();
+
+    const int nb = p.nb, nb2 = nb * nb;
+    const int sh = p.s;
+    const unsigned pm = (1u << sh) - 1u;
+    const unsigned lt_mask = (1u << lane) - 1u, le_mask = (2u << lane) - 1u;
+    unsigned long long budget = 0;       // upper bound of the hits this warp added since it last flushed
+    // previous hub of this group (its table entries are cleared before the next one is set)
+    const int32_t *prev_gi = nullptr;
+    int prev_n = 0;
+
+    int s_cur = 0, s_end = 0;
+    for (;;) {
+        if (s_cur >= s_end) {
+            int s0;
+            if (G == 1) {
+                s0 = (lane == 0) ? (int)atomicAdd(hub_counter, (unsigned)p.hub_batch) : 0;
+                s0 = __shfl_sync(0xffffffffu, s0, 0);
+            } else {
+                if (gw == 0 && lane == 0) s_fetch[group] = (int)atomicAdd(hub_counter, (unsigned)p.hub_batch);
+                group_sync<G>(group);
+                s0 = s_fetch[group];
+                group_sync<G>(group);
+            }
+            s_cur = v.s_lo + s0;
+            s_end = min(s_cur + p.hub_batch, v.s_hi);
+            if (s_cur >= v.s_hi) break;
+        }
+        const int32_t i = v.order[s_cur++];
+        const bool mine = (i >= v.h_lo && i < v.h_hi);
+        const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
+        const int n = (int)(re - rb);
+        if (n < 2) continue;
+        const int32_t *gi = v.idx_h + (rb - v.e0_h);
+        const uint8_t *gb = v.bin_h + (rb - v.e0_h);
+        const int32_t base = gi[0];
+        const unsigned span = (unsigned)(gi[n - 1] - base);
+
+        // ---- table: clear the previous hub's entries, set this hub's (warp 0 of the group) ----
+        group_sync<G>(group);                       // every warp is done looking things up
+        if (gw == 0) {
+            if (prev_n) {
+                const int32_t pbase = prev_gi[0];
+                int cbase = 0, carry = -1;
+                for (int t0 = 0; t0 < prev_n; t0 += 32) {
+                    const int t = t0 + lane;
+                    const bool ok = t < prev_n;
+                    const int d = ok ? prev_gi[t] - pbase : 0;
+                    const int g = d >> sh;
+                    int pg = __shfl_up_sync(0xffffffffu, g, 1);
+                    if (lane == 0) pg = carry;
+                    const unsigned m = __ballot_sync(0xffffffffu, ok && g != pg);
+                    const int ch = cbase + __popc(m & le_mask);
+                    if (ok) { tab[((unsigned)ch << sh) | ((unsigned)d & pm)] = (slot_t)EMPTY; pt[g] = 0; }
+                    cbase += __popc(m);
+                    carry = __shfl_sync(0xffffffffu, g, 31);
+                }
+                __syncwarp();
+            }
+            int cbase = 0, carry = -1;
+            for (int t0 = 0; t0 < n; t0 += 32) {
+                const int t = t0 + lane;
+                const bool ok = t < n;
+                const int d = ok ? gi[t] - base : 0;
+                const int g = d >> sh;
+                int pg = __shfl_up_sync(0xffffffffu, g, 1);
+                if (lane == 0) pg = carry;
+                const bool np = ok && g != pg;
+                const unsigned m = __ballot_sync(0xffffffffu, np);
+                const int ch = cbase + __popc(m & le_mask);          // chunks are numbered from 1
+                if (np) pt[g] = (uint16_t)ch;
+                if (ok) tab[((unsigned)ch << sh) | ((unsigned)d & pm)] = WEIGHTED ? (slot_t)t : (slot_t)gb[t];
+                cbase += __popc(m);
+                carry = __shfl_sync(0xffffffffu, g, 31);
+            }
+        }
+        if (WEIGHTED)
+            for (int t = gw * 32 + lane; t < n; t += G * 32) { a_w[t] = v.w[gi[t]]; a_bin[t] = gb[t]; }
+        prev_gi = gi;
+        prev_n = n;
+        group_sync<G>(group);
+
+        const double wi = WEIGHTED ? v.w[i] : 1.0;
+        // ---- blocks of 32 spokes, rows walked as one flat index space ----
+        for (int a0 = gw * 32; a0 < n - 1; a0 += G * 32) {
+            const int a = a0 + lane;
+            int nj = 0, hb = 0;
+            int64_t jb = 0;
+            double wia = 0.0;
+            if (a < n - 1) {
+                const int32_t j = gi[a];
+                if (j >= v.c_lo && j < v.c_hi) {              // foreign spokes are skipped
+                    jb = v.ptr[j];
+                    nj = (int)(v.ptr[j + 1] - jb);
+                }
+                hb = (int)gb[a] * nb2;
+                if (WEIGHTED) wia = wi * a_w[a];
+            }
+            const unsigned nz = __ballot_sync(0xffffffffu, nj > 0);
+            const int m = __popc(nz);
+            if (m == 0) continue;
+            int incl = nj;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            __syncwarp();
+            if (nj > 0) {
+                const int r = __popc(nz & lt_mask);
+                s_base[r] = (long long)(jb - v.e0_c) - (long long)(incl - nj);
+                s_hb[r] = hb;
+                s_off[r] = incl - nj;
+                if (WEIGHTED) s_wia[r] = wia;
+            }
+            __syncwarp();
+            const int myoff = (lane < m) ? s_off[lane] : INT32_MAX;
+            budget += (unsigned long long)total;
+
+            int cum = 0;
+            // U windows of 32 elements per trip: all U index loads are issued before the first look-up
+            constexpr int U = 4;
+            for (int f0 = 0; f0 < total; f0 += 32 * U) {
+                int32_t kk[U];
+                unsigned gam[U];
+                int sp[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int fu = f0 + 32 * u;
+                    kk[u] = base - 1;                      // d = 0xffffffff > span: never a member
+                    gam[u] = 0;
+                    sp[u] = 0;
+                    if (fu < total) {
+                        const int rel = myoff - fu;
+                        const unsigned sm = __reduce_or_sync(0xffffffffu, (rel >= 0 && rel < 32) ? (1u << rel) : 0u);
+                        sp[u] = cum + __popc(sm & le_mask) - 1;
+                        cum += __popc(sm);
+                        if (fu + lane < total) {
+                            const long long ad = s_base[sp[u]] + fu + lane;
+                            kk[u] = v.idx_c[ad];
+                            gam[u] = v.bin_c[ad];
+                        }
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const unsigned d = (unsigned)(kk[u] - base);
+                    if (d <= span) {
+                        const unsigned ch = pt[d >> sh];
+                        const unsigned e = tab[(ch << sh) | (d & pm)];
+                        if (e != EMPTY) {
+                            if (WEIGHTED) {
+                                const int h = s_hb[sp[u]] + (int)a_bin[e] * nb + (int)gam[u];
+                                if (p.want_counts) atomicAdd(&hist[h], 1u);
+                                atomicAdd(&my_w[h], s_wia[sp[u]] * a_w[e]);
+                            } else {
+                                atomicAdd(&hist[s_hb[sp[u]] + (int)e * nb + (int)gam[u]], 1u);
+                            }
+                        }
+                    }
+                }
+            }
+            // uint32 bins cannot wrap: any bin holds at most the hits all 8 warps added since their own last
+            // flush, and a warp flushes (atomicExch, safe against concurrent adds) before it passes 2^28
+            if (budget > (1ull << 28)) {
+                for (int t = lane; t < p.nh; t += 32) {
+                    const uint32_t c = atomicExch(&hist[t], 0u);
+                    if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
+                }
+                budget = 0;
+            }
+        }
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) {
+        const uint32_t c = hist[t];
+        if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
+    }
+}
+
 // ---- A10 fold: raw hub-ordered (b_ij, b_ik, b_jk) -> sorted triple (A-5); also sums the weight slots ------
 __global__ void k_fold3(int nb, const unsigned long long *__restrict__ raw_cnt, const double *__restrict__ raw_w,
                         int n_slots, unsigned long long *__restrict__ out_cnt, double *__restrict__ out_w)
@@ -223,24 +471,66 @@ __global__ void k_work(GrView v, unsigned long long *__restrict__ out)
 
 struct Q3Run {
     Q3Params p;
+    T3Params t;
     unsigned int *counter;
     unsigned long long *raw_cnt;
     double *raw_w;
     int grid;
     size_t smem;
-    int algo;
+    int use_table, G;
 };
+
+template <bool W>
+void launch_table(const Q3Run *r, const GrView &v, cudaStream_t st)
+{
+    switch (r->G) {
+        case 1: k_3pcf_table<W, 1><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        case 2: k_3pcf_table<W, 2><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        case 4: k_3pcf_table<W, 4><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        default: k_3pcf_table<W, 8><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+    }
+}
+
+template <bool W>
+const void *table_fn(int G)
+{
+    switch (G) {
+        case 1: return (const void *)k_3pcf_table<W, 1>;
+        case 2: return (const void *)k_3pcf_table<W, 2>;
+        case 4: return (const void *)k_3pcf_table<W, 4>;
+        default: return (const void *)k_3pcf_table<W, 8>;
+    }
+}
 
 void tile_3pcf(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
 {
     Q3Run *r = (Q3Run *)user;
     GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
-    if (r->p.weighted)
+    if (r->use_table) {
+        if (r->p.weighted) launch_table<true>(r, v, st);
+        else launch_table<false>(r, v, st);
+    } else if (r->p.weighted)
         k_3pcf_bsearch<true><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
     else
         k_3pcf_bsearch<false><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
     GR_CUDA(cudaGetLastError());
     g->n_launches += 1;
+}
+
+// shared memory of one group of the slot-table kernel for page shift s (0 = does not apply)
+size_t table_group_bytes(const gramsci_graph *g, int s, bool weighted, int G, int row_cap, int *pt_len, int *tab_len)
+{
+    const size_t a16 = 15;
+    const int64_t ptl = ((int64_t)g->max_span >> s) + 1;
+    const int64_t tbl = ((int64_t)g->max_pages[s] + 1) << s;
+    if (ptl > (1 << 20) || tbl > (1 << 20) || g->max_pages[s] >= 65535) return 0;
+    *pt_len = (int)ptl;
+    *tab_len = (int)tbl;
+    size_t b = (size_t)G * 32 * (8 + 4 + 4 + (weighted ? 8 : 0));
+    b += ((size_t)ptl * 2 + a16) & ~a16;
+    b += ((size_t)tbl * (weighted ? 2 : 1) + a16) & ~a16;
+    if (weighted) b += (size_t)row_cap * 8 + (((size_t)row_cap + a16) & ~a16);
+    return (b + a16) & ~a16;
 }
 
 struct Q2Run { unsigned long long *cnt; double *w; int weighted; };
@@ -275,27 +565,70 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     GrTimer total(st);
     g->n_launches = 0;
     g->staged_bytes = 0;
+    if (!d_counts && !d_wsum) { g->t_query_ms = total.stop(); return; }
 
     Q3Run r;
-    r.algo = g->algo;
     r.p.nb = nb; r.p.nh = nh;
     r.p.weighted = (d_wsum != nullptr) ? 1 : 0;
     r.p.want_counts = (d_counts != nullptr) ? 1 : 0;
     r.p.row_cap = std::max(16, (g->max_row + 15) & ~15);
-    r.p.smem_hist = ((size_t)nh * 4 <= 96 * 1024) ? 1 : 0;
-    size_t per_entry = 4 + 1 + (r.p.weighted ? 8 : 0);
-    r.smem = (size_t)r.p.row_cap * per_entry + (r.p.smem_hist ? (size_t)nh * 4 : 0) + 64;
-    if (r.smem > g->smem_optin)
-        GR_FAIL(GRAMSCI_ERANGE, "3pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
-    GR_CUDA(cudaFuncSetAttribute(k_3pcf_bsearch<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r.smem));
-    GR_CUDA(cudaFuncSetAttribute(k_3pcf_bsearch<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r.smem));
+    const bool W = r.p.weighted != 0;
+
+    // ---- slot-table kernel: page shift s minimising the table, then the smallest group that fits ----
+    r.use_table = 0;
+    r.G = 8;
+    if (g->algo != GRAMSCI_ALGO_BSEARCH && g->max_row >= 2 && g->max_row < 65535) {
+        const size_t hist_bytes = (((size_t)nh * 4 + 15) & ~(size_t)15) + 16;
+        int best_s = -1, ptl = 0, tbl = 0;
+        size_t best = 0;
+        for (int s = GR_S_MIN; s <= GR_S_MAX; ++s) {
+            int a = 0, b = 0;
+            const size_t bytes = table_group_bytes(g, s, W, 1, r.p.row_cap, &a, &b);
+            if (bytes && (best_s < 0 || bytes < best)) { best = bytes; best_s = s; ptl = a; tbl = b; }
+        }
+        if (best_s >= 0) {
+            const size_t soft = 100 * 1024;       // two CTAs per SM
+            int G = 0;
+            const int forced = (g->algo >= GRAMSCI_ALGO_TABLE_G1) ? (1 << (g->algo - GRAMSCI_ALGO_TABLE_G1)) : 0;
+            for (int cand = 1; cand <= 8 && !G; cand *= 2) {
+                if (forced && cand != forced) continue;
+                const size_t cta = hist_bytes + (size_t)(Q3_WARPS / cand) * table_group_bytes(g, best_s, W, cand, r.p.row_cap, &ptl, &tbl);
+                if (cta <= soft || ((cand == 8 || forced) && cta <= g->smem_optin)) G = cand;
+            }
+            if (G) {
+                r.use_table = 1;
+                r.G = G;
+                r.t.nb = nb; r.t.nh = nh; r.t.s = best_s; r.t.pt_len = ptl; r.t.tab_len = tbl;
+                r.t.row_cap = r.p.row_cap; r.t.want_counts = r.p.want_counts;
+                r.t.group_bytes = (int)table_group_bytes(g, best_s, W, G, r.p.row_cap, &ptl, &tbl);
+                r.t.hub_batch = (G == 8) ? 1 : 4;
+                r.smem = hist_bytes + (size_t)(Q3_WARPS / G) * r.t.group_bytes;
+            }
+        }
+        if (!r.use_table && g->algo >= GRAMSCI_ALGO_BITMAP)
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table does not fit in shared memory (span %d, row %d)", g->max_span, g->max_row);
+    }
+    const void *fn;
+    if (r.use_table) {
+        fn = W ? table_fn<true>(r.G) : table_fn<false>(r.G);
+    } else {
+        r.p.smem_hist = ((size_t)nh * 4 <= 96 * 1024) ? 1 : 0;
+        size_t per_entry = 4 + 1 + (W ? 8 : 0);
+        r.smem = (size_t)r.p.row_cap * per_entry + (r.p.smem_hist ? (size_t)nh * 4 : 0) + 64;
+        if (r.smem > g->smem_optin)
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
+        fn = W ? (const void *)k_3pcf_bsearch<true> : (const void *)k_3pcf_bsearch<false>;
+    }
+    GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r.smem));
     int occ = 1;
-    if (r.p.weighted)
-        GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_3pcf_bsearch<true>, Q3_THREADS, r.smem));
-    else
-        GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_3pcf_bsearch<false>, Q3_THREADS, r.smem));
+    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, Q3_THREADS, r.smem));
     occ = std::max(1, std::min(occ, 8));
     r.grid = g->sm_count * occ;
+
+    if (getenv("GRAMSCI_DEBUG"))
+        fprintf(stderr, "[gramsci] 3pcf: table=%d G=%d s=%d pt_len=%d tab_len=%d group_bytes=%d smem=%zu occ=%d grid=%d span=%d row=%d\n",
+                r.use_table, r.G, r.use_table ? r.t.s : -1, r.use_table ? r.t.pt_len : 0, r.use_table ? r.t.tab_len : 0,
+                r.use_table ? r.t.group_bytes : 0, r.smem, occ, r.grid, g->max_span, g->max_row);
 
     DevBuf<unsigned int> counter;
     DevBuf<unsigned long long> raw_cnt;
@@ -303,9 +636,10 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     counter.alloc(1);
     raw_cnt.alloc((size_t)nh);
     GR_CUDA(cudaMemsetAsync(raw_cnt.p, 0, sizeof(unsigned long long) * nh, st));
-    if (r.p.weighted) {
-        raw_w.alloc((size_t)nh * r.grid);
-        GR_CUDA(cudaMemsetAsync(raw_w.p, 0, sizeof(double) * (size_t)nh * r.grid, st));
+    const int n_slots = r.grid;                         // one fp64 slab per CTA
+    if (W) {
+        raw_w.alloc((size_t)nh * n_slots);
+        GR_CUDA(cudaMemsetAsync(raw_w.p, 0, sizeof(double) * (size_t)nh * n_slots, st));
     }
     r.counter = counter.p; r.raw_cnt = raw_cnt.p; r.raw_w = raw_w.p;
 
@@ -314,7 +648,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         gr_for_each_tile(g, false, false, tile_3pcf, &r);
         g->t_enum_ms = en.stop();
     }
-    k_fold3<<<(nh + 255) / 256, 256, 0, st>>>(nb, raw_cnt.p, r.p.weighted ? raw_w.p : nullptr, r.grid,
+    k_fold3<<<(nh + 255) / 256, 256, 0, st>>>(nb, d_counts ? raw_cnt.p : nullptr, W ? raw_w.p : nullptr, n_slots,
                                              (unsigned long long *)d_counts, d_wsum);
     GR_CUDA(cudaGetLastError());
     g->n_launches += 1;

@@ -73,7 +73,10 @@ def test_2pcf(relabel):
     assert_weighted_close(w, ow)
 
 
-@pytest.mark.parametrize("algo", [gr.ALGO_BSEARCH])
+ALGOS = [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G1, gr.ALGO_TABLE_G2, gr.ALGO_TABLE_G4, gr.ALGO_TABLE_G8]
+
+
+@pytest.mark.parametrize("algo", ALGOS)
 @pytest.mark.parametrize("relabel", [1, 2])
 def test_3pcf_config1(relabel, algo):
     cfg = cat.config1()
@@ -87,7 +90,7 @@ def test_3pcf_config1(relabel, algo):
     assert np.array_equal(c2, oc)
 
 
-@pytest.mark.parametrize("algo", [gr.ALGO_BSEARCH])
+@pytest.mark.parametrize("algo", ALGOS)
 @pytest.mark.parametrize("periodic,r_min", [(True, 0.0), (False, 0.0), (True, 2.0)])
 def test_3pcf_weighted(periodic, r_min, algo):
     cfg = small(13, n=4000, L=40.0, weighted=True, periodic=periodic, r_min=r_min, nb=7)
@@ -211,3 +214,70 @@ def test_4pcf_edge_cases():
     assert c.sum() == 1 and c[0] == 1
     with pytest.raises(gr.GramsciError):
         gr.gramsci_build_graph(tet, None, None, 0.0, 3.0, 17).pcf4()
+
+
+# ---- larger / clustered shapes and the out-of-core tiler (S:8(a) A11; pin C-13) -----------------------------
+@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4])
+def test_3pcf_clustered_replica(algo):
+    """1/64 replica of BASELINE configs[1] data (Neyman-Scott, same densities, fp64 weights)."""
+    cfg = cat.config2_data(seed=2101, n=15_625, L=250.0, mean_parents=156.25)
+    og, gg = build_both(cfg, algo=algo)
+    oc, ow = og.pcf3()
+    c, w = gg.pcf3(weighted=True)
+    assert c.sum() > 5e6
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+
+
+_BAO = {}
+
+
+def _bao_replica():
+    if not _BAO:
+        cfg = cat.config5(seed=5101, n=6_000, L=310.0)
+        og = oracle.Graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+        _BAO["cfg"], _BAO["cnt"] = cfg, og.pcf3()[0]
+    return _BAO["cfg"], _BAO["cnt"]
+
+
+@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH])
+def test_3pcf_bao_replica(algo):
+    """Shrunk replica of BASELINE configs[4] (same radii and bins, L=310, 40 % of the density so that
+    the oracle finishes in seconds): rows of thousands of entries, r_min > 0, 18 bins, a periodic grid
+    with two cells per axis."""
+    cfg, oc = _bao_replica()
+    gg = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], algo=algo)
+    c, _ = gg.pcf3()
+    assert gg.info()["max_row"] > 2000 and oc.sum() > 1e9
+    assert np.array_equal(c, oc)
+
+
+@pytest.mark.parametrize("relabel", [1, 2])
+@pytest.mark.parametrize("n_windows,cap_frac", [(2, 1.2), (5, 1.0), (7, 0.45)])
+def test_out_of_core_equals_in_core(relabel, n_windows, cap_frac):
+    """C-13: the capped (windowed, streamed from pinned host memory) run is bit-identical to the in-core
+    run for any window count, including windows forced small on a tiny input."""
+    cfg = small(31, n=6000, L=40.0, weighted=True, r_max=5.0, nb=5)
+    og, g0 = build_both(cfg, relabel=relabel)
+    oc, ow = og.pcf3()
+    csr = g0.info()["csr_bytes"]
+    _, g1 = build_both(cfg, relabel=relabel, device_mem_cap_bytes=int(csr * cap_frac), n_windows=n_windows)
+    assert g1.info()["n_windows"] == n_windows and g1.info()["n_edges"] == og.n_edges
+    c, w = g1.pcf3(weighted=True)
+    assert np.array_equal(c, oc)
+    assert np.array_equal(c, g0.pcf3()[0])
+    assert_weighted_close(w, ow)
+    assert g1.timing(4) >= csr * 0.99            # every window was staged at least once
+    c2, w2 = g1.pcf2(weighted=True)
+    assert np.array_equal(c2, og.pcf2()[0])
+
+
+def test_out_of_core_cap_derives_windows():
+    cfg = small(32, n=8000, L=40.0, r_max=5.0, nb=4)
+    og, g0 = build_both(cfg)
+    csr = g0.info()["csr_bytes"]
+    _, g1 = build_both(cfg, device_mem_cap_bytes=csr // 2)
+    assert g1.info()["n_windows"] >= 8           # four window buffers must fit under the cap
+    assert np.array_equal(g1.pcf3()[0], og.pcf3()[0])
+    with pytest.raises(gr.GramsciError):
+        g1.pcf4()
