@@ -30,6 +30,32 @@ extern "C" const char *gramsci_last_error(void) { return t_err; }
     catch (...) { gr_set_error("unexpected internal error"); return GRAMSCI_ECUDA; }                  \
     return GRAMSCI_OK;
 
+// ---- allocation stream / pools ---------------------------------------------------------------------------
+cudaStream_t &gr_alloc_stream()
+{
+    static thread_local cudaStream_t st = nullptr;
+    return st;
+}
+
+bool gr_pools_supported()
+{
+    static int state = -1;                 // -1 unknown, 0 no, 1 yes
+    if (state < 0) {
+        int dev = 0, ok = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&ok, cudaDevAttrMemoryPoolsSupported, dev) == cudaSuccess && ok) {
+            cudaMemPool_t pool;
+            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                uint64_t thr = UINT64_MAX;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+                state = 1;
+            }
+        }
+        if (state < 0) { state = 0; cudaGetLastError(); }
+    }
+    return state == 1;
+}
+
 // ---- pointer staging -------------------------------------------------------------------------------------
 static bool is_device_ptr(const void *p)
 {
@@ -146,6 +172,7 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->sm_count = prop.multiProcessorCount;
     g->smem_optin = prop.sharedMemPerBlockOptin;
 
+    gr_alloc_stream() = g->stream;
     DevBuf<double> hp, hw;
     const double *d_pts = stage_in(points, (size_t)N * 3, hp, g->stream);
     const double *d_w = stage_in(weights, (size_t)N, hw, g->stream);
@@ -163,6 +190,7 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
 extern "C" void gramsci_free_graph(gramsci_graph *g)
 {
     if (!g) return;
+    cudaStreamSynchronize(g->stream);
     if (g->h_idx) cudaFreeHost(g->h_idx);
     if (g->h_bin) cudaFreeHost(g->h_bin);
     if (g->h_pix) cudaFreeHost(g->h_pix);
@@ -186,6 +214,7 @@ extern "C" int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t 
 {
     GR_API_BEGIN
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "export_csr: NULL graph");
+    gr_alloc_stream() = g->stream;
     OutStage<int64_t> op; OutStage<int32_t> oi; OutStage<uint8_t> ob, ox;
     op.init(ptr, (size_t)g->n + 1);
     oi.init(idx, (size_t)g->n_edges);
@@ -202,6 +231,7 @@ extern "C" int gramsci_2pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "2pcf: NULL graph");
+    gr_alloc_stream() = g->stream;
     OutStage<uint64_t> oc; OutStage<double> ow;
     oc.init(counts, (size_t)g->nb);
     ow.init(wsum, (size_t)g->nb);
@@ -215,6 +245,7 @@ extern "C" int gramsci_3pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "3pcf: NULL graph");
+    gr_alloc_stream() = g->stream;
     const size_t nh = (size_t)ipow(g->nb, 3);
     OutStage<uint64_t> oc; OutStage<double> ow;
     oc.init(counts, nh);
@@ -229,6 +260,7 @@ extern "C" int gramsci_4pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "4pcf: NULL graph");
+    gr_alloc_stream() = g->stream;
     if (g->nb > 16) GR_FAIL(GRAMSCI_EINVAL, "4pcf: nbins must be <= 16");
     const size_t nh = (size_t)ipow(g->nb, 6);
     OutStage<uint64_t> oc; OutStage<double> ow;
@@ -245,6 +277,7 @@ extern "C" int gramsci_4pcf_parity(const gramsci_graph *cg, uint64_t *even_count
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: NULL graph");
+    gr_alloc_stream() = g->stream;
     if (g->nb > 16) GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: nbins must be <= 16");
     if (!g->has_pix || g->spatial)
         GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: graph must be built with want_pixels=1 in caller-label order (A-10)");
@@ -279,6 +312,7 @@ extern "C" int gramsci_work_counters(const gramsci_graph *cg, uint64_t *spoke_el
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "work_counters: NULL graph");
+    gr_alloc_stream() = g->stream;
     gr_work_counters(g, spoke_elems, tail_elems);
     GR_API_END
 }

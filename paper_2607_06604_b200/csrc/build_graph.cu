@@ -444,40 +444,76 @@ __global__ void k_export_fill(const int64_t *__restrict__ ptr, const int32_t *__
 }
 
 // ---- row statistics for the slot-table 3pCF kernel: one warp per row -------------------------------------
-// out[0] = max over rows of (last - first); out[1 + s - GR_S_MIN] = max over rows of the number of
-// distinct pages ((k - first) >> s) among the row's entries.  Rows are sorted, so a page starts where
-// an entry's page differs from its predecessor's.
+// The kernel keys its table by d(k) = k - first, after cutting the LARGEST gap between consecutive entries
+// out of the row (rows of hubs next to a periodic face reach labels at the other end of the label range):
+// entries before the gap keep d = k - first, entries from `brk` (first entry after the gap) on get
+// d = k - brk + off(s), off(s) = two pages past the page of the last entry before the gap (one guard page).
+// For every page shift s this emits   out[2*(s-GR_S_MIN)]   = max over rows of the page-table length
+//                                     out[2*(s-GR_S_MIN)+1] = max over rows of the number of touched pages.
 __global__ void __launch_bounds__(256)
 k_row_stats(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, int64_t e0, int32_t row_lo,
             int32_t row_hi, int32_t *__restrict__ out)
 {
+    __shared__ int s_max[2 * (GR_S_MAX - GR_S_MIN + 1)];
+    if (threadIdx.x < 2 * (GR_S_MAX - GR_S_MIN + 1)) s_max[threadIdx.x] = 0;
+    __syncthreads();
     const int lane = threadIdx.x & 31;
     const int64_t r = row_lo + ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / 32;
-    if (r >= row_hi) return;
-    const int64_t b = ptr[r] - e0, e = ptr[r + 1] - e0;
-    if (e - b < 1) return;
+    int64_t b = 0, e = 0;
+    if (r < row_hi) { b = ptr[r] - e0; e = ptr[r + 1] - e0; }
+    if (e - b >= 2) {
     const int32_t first = idx[b], last = idx[e - 1];
+    // pass 1: first largest gap
+    int best_gap = 0;
+    int64_t best_t = b + 1;
+    int32_t carry = first;
+    for (int64_t t0 = b; t0 < e; t0 += 32) {
+        const int64_t t = t0 + lane;
+        const int32_t k = (t < e) ? idx[t] : 0;
+        int32_t prev = __shfl_up_sync(0xffffffffu, k, 1);
+        if (lane == 0) prev = carry;
+        const int gap = (t < e) ? k - prev : 0;
+        const int m = __reduce_max_sync(0xffffffffu, gap);
+        if (m > best_gap) {
+            best_gap = m;
+            best_t = t0 + __ffs(__ballot_sync(0xffffffffu, gap == m)) - 1;
+        }
+        carry = __shfl_sync(0xffffffffu, k, 31);
+    }
+    const int32_t lowmax = idx[best_t - 1], brk = idx[best_t];
+    // pass 2: touched pages per shift
     int cnt[GR_S_MAX - GR_S_MIN + 1];
 #pragma unroll
     for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) cnt[s] = 0;
-    int32_t carry = -1;                        // d of the previous chunk's last entry
+    int32_t cprev = -1;      // previous entry (label), -1 = none
     for (int64_t t0 = b; t0 < e; t0 += 32) {
         const int64_t t = t0 + lane;
-        const int32_t d = (t < e) ? idx[t] - first : 0;
-        int32_t prev = __shfl_up_sync(0xffffffffu, d, 1);
-        if (lane == 0) prev = carry;
+        const bool ok = t < e;
+        const int32_t k = ok ? idx[t] : 0;
+        int32_t prev = __shfl_up_sync(0xffffffffu, k, 1);
+        if (lane == 0) prev = cprev;
 #pragma unroll
         for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) {
-            const bool np = (t < e) && (prev < 0 || (d >> (s + GR_S_MIN)) != (prev >> (s + GR_S_MIN)));
-            cnt[s] += __popc(__ballot_sync(0xffffffffu, np));
+            const int sh = s + GR_S_MIN;
+            // page identity: (side of the gap, page inside that side)
+            const int pk = (k >= brk) ? (((k - brk) >> sh) | 0x40000000) : ((k - first) >> sh);
+            const int pp = (prev < 0) ? -1 : ((prev >= brk) ? (((prev - brk) >> sh) | 0x40000000) : ((prev - first) >> sh));
+            cnt[s] += __popc(__ballot_sync(0xffffffffu, ok && pk != pp));
         }
-        carry = __shfl_sync(0xffffffffu, d, 31);
+        cprev = __shfl_sync(0xffffffffu, k, 31);
     }
     if (lane == 0) {
-        atomicMax(&out[0], last - first);
 #pragma unroll
-        for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) atomicMax(&out[1 + s], cnt[s]);
+        for (int s = 0; s <= GR_S_MAX - GR_S_MIN; ++s) {
+            const int sh = s + GR_S_MIN;
+            const int ptl = ((lowmax - first) >> sh) + 2 + ((last - brk) >> sh) + 1;   // low pages, guard, high pages
+            atomicMax(&s_max[2 * s], ptl);
+            atomicMax(&s_max[2 * s + 1], cnt[s]);
+        }
     }
+    }
+    __syncthreads();      // one global atomic per block and value, not per row (same-address atomics serialise in L2)
+    if (threadIdx.x < 2 * (GR_S_MAX - GR_S_MIN + 1) && s_max[threadIdx.x] > 0) atomicMax(&out[threadIdx.x], s_max[threadIdx.x]);
 }
 
 // largest neighbour label stored in edges [lo,hi) (which search windows a hub window reaches; tiler.cu)
@@ -696,8 +732,8 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     }
 
     DevBuf<int32_t> stats;
-    stats.alloc(16);
-    GR_CUDA(cudaMemsetAsync(stats.p, 0, sizeof(int32_t) * 16, st));
+    stats.alloc(32);
+    GR_CUDA(cudaMemsetAsync(stats.p, 0, sizeof(int32_t) * 32, st));
 
     // --- A4 fill (+ A5 sort when labels are not in cell order) per window ---
     if (!g->ooc) {
@@ -763,11 +799,13 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         }
     }
     {
-        int32_t h[16];
+        int32_t h[32];
         GR_CUDA(cudaMemcpyAsync(h, stats.p, sizeof h, cudaMemcpyDeviceToHost, st));
         GR_CUDA(cudaStreamSynchronize(st));
-        g->max_span = h[0];
-        for (int s = GR_S_MIN; s <= GR_S_MAX; ++s) g->max_pages[s] = h[1 + s - GR_S_MIN];
+        for (int s = GR_S_MIN; s <= GR_S_MAX; ++s) {
+            g->max_ptl[s] = h[2 * (s - GR_S_MIN)];
+            g->max_pages[s] = h[2 * (s - GR_S_MIN) + 1];
+        }
     }
     g->t_build_ms = timer.stop();
     g->n_launches = launches;

@@ -33,10 +33,20 @@ struct GrFail { int code; };   // thrown inside the library only; every ABI entr
     } while (0)
 
 // ---- device buffer owned by the library --------------------------------------------------------
+// Stream-ordered allocations (cudaMallocAsync from the device's default pool, release threshold raised
+// so that freed blocks are reused by the next call instead of going back to the driver): a graph build
+// or a query allocates tens of scratch buffers and must not pay a device synchronisation for each.
+// Every ABI entry sets the stream its buffers are ordered on (gr_alloc_stream); all library work
+// runs on that stream.
+cudaStream_t &gr_alloc_stream();
+bool gr_pools_supported();
+
 template <typename T>
 struct DevBuf {
     T *p = nullptr;
     size_t n = 0;
+    cudaStream_t st = nullptr;
+    bool async = false;
     DevBuf() {}
     DevBuf(const DevBuf &) = delete;
     DevBuf &operator=(const DevBuf &) = delete;
@@ -46,10 +56,16 @@ struct DevBuf {
         n = count;
         size_t bytes = (count ? count : 1) * sizeof(T);
         bytes = (bytes + 255) & ~size_t(255);          // tail padding: aligned vector loads may over-read
-        GR_CUDA(cudaMalloc((void **)&p, bytes + 256));
+        async = gr_pools_supported();
+        st = gr_alloc_stream();
+        if (async) GR_CUDA(cudaMallocAsync((void **)&p, bytes + 256, st));
+        else GR_CUDA(cudaMalloc((void **)&p, bytes + 256));
     }
     void release() {
-        if (p) cudaFree(p);
+        if (p) {
+            if (async) cudaFreeAsync(p, st);
+            else cudaFree(p);
+        }
         p = nullptr;
         n = 0;
     }
@@ -85,9 +101,9 @@ struct gramsci_graph {
     DevBuf<double> w;              // [n] weights by internal label
     DevBuf<int32_t> order;         // [n] label at spatial slot s
     DevBuf<int32_t> caller_of;     // [n] caller label of internal label (spatial mode), else empty
-    // row statistics for the slot-table 3pCF kernel (query3.cu): label span of a row (last - first) and,
-    // for page size 2^s labels (s = GR_S_MIN .. GR_S_MAX), the number of distinct pages a row touches
-    int32_t max_span = 0;
+    // row statistics for the slot-table 3pCF kernel (query3.cu; k_row_stats in build_graph.cu): for page
+    // size 2^s labels (s = GR_S_MIN .. GR_S_MAX), the longest page table and the most pages a row touches
+    int32_t max_ptl[16] = {0};
     int32_t max_pages[16] = {0};
     // out-of-core state: edge arrays in pinned host memory, cut into row-aligned windows
     uint64_t cap_bytes = 0;

@@ -219,11 +219,18 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
     const int nb = p.nb, nb2 = nb * nb;
     const int sh = p.s;
     const unsigned pm = (1u << sh) - 1u;
+    const unsigned ptl1 = (unsigned)p.pt_len - 1u;       // sentinel page: always chunk 0 (all EMPTY)
     const unsigned lt_mask = (1u << lane) - 1u, le_mask = (2u << lane) - 1u;
     unsigned long long budget = 0;       // upper bound of the hits this warp added since it last flushed
+    // key of a label k in the current hub's table: the largest gap of the row is cut out (rows next to a
+    // periodic face reach the far end of the label range):
+    //   k <  brk : d = min(k - base, guard)      (labels inside the gap land on the empty guard page)
+    //   k >= brk : d = k - brk + off,  off = guard + 2^s
     // previous hub of this group (its table entries are cleared before the next one is set)
     const int32_t *prev_gi = nullptr;
     int prev_n = 0;
+    int32_t prev_base = 0, prev_brk = 0;
+    unsigned prev_off = 0;
 
     int s_cur = 0, s_end = 0;
     for (;;) {
@@ -250,24 +257,47 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
         const int32_t *gi = v.idx_h + (rb - v.e0_h);
         const uint8_t *gb = v.bin_h + (rb - v.e0_h);
         const int32_t base = gi[0];
-        const unsigned span = (unsigned)(gi[n - 1] - base);
+        // first largest gap of the row (every warp of the group computes the same values)
+        int32_t brk, lowmax;
+        {
+            int best_gap = 0, best_t = 1;
+            int32_t carry = base;
+            for (int t0 = 0; t0 < n; t0 += 32) {
+                const int t = t0 + lane;
+                const int32_t k = (t < n) ? gi[t] : 0;
+                int32_t pk = __shfl_up_sync(0xffffffffu, k, 1);
+                if (lane == 0) pk = carry;
+                const int gap = (t < n) ? k - pk : 0;
+                const int m = __reduce_max_sync(0xffffffffu, gap);
+                if (m > best_gap) {
+                    best_gap = m;
+                    best_t = t0 + __ffs(__ballot_sync(0xffffffffu, gap == m)) - 1;
+                }
+                carry = __shfl_sync(0xffffffffu, k, 31);
+            }
+            lowmax = gi[best_t - 1];
+            brk = gi[best_t];
+        }
+        const unsigned guard = ((((unsigned)(lowmax - base)) >> sh) + 1u) << sh;
+        const unsigned off = guard + (1u << sh);
+        const int32_t sub_hi = brk - (int32_t)off;
 
         // ---- table: clear the previous hub's entries, set this hub's (warp 0 of the group) ----
         group_sync<G>(group);                       // every warp is done looking things up
         if (gw == 0) {
             if (prev_n) {
-                const int32_t pbase = prev_gi[0];
                 int cbase = 0, carry = -1;
                 for (int t0 = 0; t0 < prev_n; t0 += 32) {
                     const int t = t0 + lane;
                     const bool ok = t < prev_n;
-                    const int d = ok ? prev_gi[t] - pbase : 0;
-                    const int g = d >> sh;
+                    const int32_t k = ok ? prev_gi[t] : prev_base;
+                    const unsigned d = (k >= prev_brk) ? (unsigned)(k - prev_brk) + prev_off : (unsigned)(k - prev_base);
+                    const int g = (int)(d >> sh);
                     int pg = __shfl_up_sync(0xffffffffu, g, 1);
                     if (lane == 0) pg = carry;
                     const unsigned m = __ballot_sync(0xffffffffu, ok && g != pg);
                     const int ch = cbase + __popc(m & le_mask);
-                    if (ok) { tab[((unsigned)ch << sh) | ((unsigned)d & pm)] = (slot_t)EMPTY; pt[g] = 0; }
+                    if (ok) { tab[((unsigned)ch << sh) | (d & pm)] = (slot_t)EMPTY; pt[g] = 0; }
                     cbase += __popc(m);
                     carry = __shfl_sync(0xffffffffu, g, 31);
                 }
@@ -277,15 +307,16 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             for (int t0 = 0; t0 < n; t0 += 32) {
                 const int t = t0 + lane;
                 const bool ok = t < n;
-                const int d = ok ? gi[t] - base : 0;
-                const int g = d >> sh;
+                const int32_t k = ok ? gi[t] : base;
+                const unsigned d = (k >= brk) ? (unsigned)(k - sub_hi) : (unsigned)(k - base);
+                const int g = (int)(d >> sh);
                 int pg = __shfl_up_sync(0xffffffffu, g, 1);
                 if (lane == 0) pg = carry;
                 const bool np = ok && g != pg;
                 const unsigned m = __ballot_sync(0xffffffffu, np);
                 const int ch = cbase + __popc(m & le_mask);          // chunks are numbered from 1
                 if (np) pt[g] = (uint16_t)ch;
-                if (ok) tab[((unsigned)ch << sh) | ((unsigned)d & pm)] = WEIGHTED ? (slot_t)t : (slot_t)gb[t];
+                if (ok) tab[((unsigned)ch << sh) | (d & pm)] = WEIGHTED ? (slot_t)t : (slot_t)gb[t];
                 cbase += __popc(m);
                 carry = __shfl_sync(0xffffffffu, g, 31);
             }
@@ -294,6 +325,9 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             for (int t = gw * 32 + lane; t < n; t += G * 32) { a_w[t] = v.w[gi[t]]; a_bin[t] = gb[t]; }
         prev_gi = gi;
         prev_n = n;
+        prev_base = base;
+        prev_brk = brk;
+        prev_off = off;
         group_sync<G>(group);
 
         const double wi = WEIGHTED ? v.w[i] : 1.0;
@@ -344,7 +378,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const int fu = f0 + 32 * u;
-                    kk[u] = base - 1;                      // d = 0xffffffff > span: never a member
+                    kk[u] = base - 1;                      // below the row: lands on the guard page, never a member
                     gam[u] = 0;
                     sp[u] = 0;
                     if (fu < total) {
@@ -361,18 +395,18 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
                 }
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
-                    const unsigned d = (unsigned)(kk[u] - base);
-                    if (d <= span) {
-                        const unsigned ch = pt[d >> sh];
-                        const unsigned e = tab[(ch << sh) | (d & pm)];
-                        if (e != EMPTY) {
-                            if (WEIGHTED) {
-                                const int h = s_hb[sp[u]] + (int)a_bin[e] * nb + (int)gam[u];
-                                if (p.want_counts) atomicAdd(&hist[h], 1u);
-                                atomicAdd(&my_w[h], s_wia[sp[u]] * a_w[e]);
-                            } else {
-                                atomicAdd(&hist[s_hb[sp[u]] + (int)e * nb + (int)gam[u]], 1u);
-                            }
+                    const int32_t k = kk[u];
+                    const bool hi = k >= brk;
+                    const unsigned d = min((unsigned)(k - (hi ? sub_hi : base)), hi ? 0xffffffffu : guard);
+                    const unsigned ch = pt[min(d >> sh, ptl1)];
+                    const unsigned e = tab[(ch << sh) | (d & pm)];
+                    if (e != EMPTY) {
+                        if (WEIGHTED) {
+                            const int h = s_hb[sp[u]] + (int)a_bin[e] * nb + (int)gam[u];
+                            if (p.want_counts) atomicAdd(&hist[h], 1u);
+                            atomicAdd(&my_w[h], s_wia[sp[u]] * a_w[e]);
+                        } else {
+                            atomicAdd(&hist[s_hb[sp[u]] + (int)e * nb + (int)gam[u]], 1u);
                         }
                     }
                 }
@@ -521,7 +555,7 @@ void tile_3pcf(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
 size_t table_group_bytes(const gramsci_graph *g, int s, bool weighted, int G, int row_cap, int *pt_len, int *tab_len)
 {
     const size_t a16 = 15;
-    const int64_t ptl = ((int64_t)g->max_span >> s) + 1;
+    const int64_t ptl = (int64_t)g->max_ptl[s] + 1;      // + sentinel page
     const int64_t tbl = ((int64_t)g->max_pages[s] + 1) << s;
     if (ptl > (1 << 20) || tbl > (1 << 20) || g->max_pages[s] >= 65535) return 0;
     *pt_len = (int)ptl;
@@ -606,7 +640,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
             }
         }
         if (!r.use_table && g->algo >= GRAMSCI_ALGO_BITMAP)
-            GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table does not fit in shared memory (span %d, row %d)", g->max_span, g->max_row);
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table does not fit in shared memory (longest row %d)", g->max_row);
     }
     const void *fn;
     if (r.use_table) {
@@ -628,7 +662,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     if (getenv("GRAMSCI_DEBUG"))
         fprintf(stderr, "[gramsci] 3pcf: table=%d G=%d s=%d pt_len=%d tab_len=%d group_bytes=%d smem=%zu occ=%d grid=%d span=%d row=%d\n",
                 r.use_table, r.G, r.use_table ? r.t.s : -1, r.use_table ? r.t.pt_len : 0, r.use_table ? r.t.tab_len : 0,
-                r.use_table ? r.t.group_bytes : 0, r.smem, occ, r.grid, g->max_span, g->max_row);
+                r.use_table ? r.t.group_bytes : 0, r.smem, occ, r.grid, 0, g->max_row);
 
     DevBuf<unsigned int> counter;
     DevBuf<unsigned long long> raw_cnt;

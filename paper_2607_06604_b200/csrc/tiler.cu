@@ -69,7 +69,15 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         GR_CUDA(cudaEventCreateWithFlags(&s.ready, cudaEventDisableTiming));
         GR_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
     }
-    // the copy stream must not start before earlier work on the compute stream (e.g. memsets) is ordered
+    // the window buffers are stream-ordered allocations on `st`: the copy stream may touch them only after
+    // that point of `st`
+    {
+        cudaEvent_t ev;
+        GR_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        GR_CUDA(cudaEventRecord(ev, st));
+        GR_CUDA(cudaStreamWaitEvent(cs, ev, 0));
+        GR_CUDA(cudaEventDestroy(ev));
+    }
     uint64_t clock = 0;
 
     // bring window `wid` into a slot (cache hit: no copy); never evicts a slot whose bit is set in `protect`
