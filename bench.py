@@ -31,6 +31,12 @@ sys.path.insert(0, ROOT)
 import catalogues as cat  # noqa: E402
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on cfg2, from the committed
+# ncu --set full capture (profiles/r1_b_table_3pcf_full.md)
+DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 578.146816e6 + 6.029568e6,
+                      "k_3pcf_table<counts>": 301.713408e6 + 4.563456e6}
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -80,6 +86,33 @@ class ClockSampler(threading.Thread):
         busy = [x for x in sm if x > 0]
         return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": mx or None,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def rank_seed_shift(rank: int) -> int:
+    """Sharding rule for N > 1: every rank runs the same workload shape on its own seeds (independent
+    catalogues, no data-path collective)."""
+    return 1000 * rank
+
+
+def max_over_ranks(value: float, device=None) -> float:
+    """Time of a multi-rank step = the slowest rank's device time (all-reduce MAX of one scalar; works on
+    the gloo backend with CPU tensors, which is how tests/test_multirank_host.py exercises it)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value: float, device=None) -> float:
+    """Whole-job units processed = sum over ranks (all-reduce SUM of one scalar)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
 
 
 def workload(name: str, seed_shift: int = 0):
@@ -167,7 +200,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gr.load_library()
 
-    cats = workload(args.workload, seed_shift=1000 * rank)
+    cats = workload(args.workload, seed_shift=rank_seed_shift(rank))
     dev = [(torch.from_numpy(c["points"]).cuda(), None if c["weights"] is None else torch.from_numpy(c["weights"]).cuda())
            for c in cats]
     pin = [(torch.from_numpy(c["points"]).pin_memory(), None if c["weights"] is None else torch.from_numpy(c["weights"]).pin_memory())
@@ -176,29 +209,33 @@ def run_ours(args):
     stats = {}
 
     def step(host: bool, count_work: bool = False):
-        """one pass of the hot path over the batch; returns (triangles, per-step stats)"""
+        """one pass of the hot path over the batch; returns (triangles, per-step stats, per-catalogue stats)"""
         tri = 0
-        st = {"enum_ms": 0.0, "build_ms": 0.0, "query_ms": 0.0, "launches": 0.0, "bytes": 0.0, "edges": 0,
-              "spoke": 0, "tail": 0}
+        st = {"enum_ms": 0.0, "build_ms": 0.0, "query_ms": 0.0, "launches": 0.0, "edges": 0}
+        per = []
         for c, d, p in zip(cats, dev, pin):
             pts, w = (p if host else d)
             g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo)
             st["build_ms"] += g.timing(0)
             st["launches"] += g.timing(3)
             cnt, ws = g.pcf3(counts=True, weighted=(w is not None), host=host)
+            pc = {"name": c["name"], "enum_ms": g.timing(2), "weighted": w is not None}
             st["enum_ms"] += g.timing(2)
             st["query_ms"] += g.timing(1)
             st["launches"] += g.timing(3)
             t = int(cnt.sum())
             tri += t
-            st["edges"] += g.info()["n_edges"]
+            e = g.info()["n_edges"]
+            st["edges"] += e
             if count_work:
                 sp, tl = g.work_counters()
-                st["spoke"] += sp
-                st["tail"] += tl
-                st["bytes"] += 4.0 * sp + 4.0 * tl + g.info()["n_edges"] + 2.0 * t
+                # algorithmic bytes of the enumeration (DESIGN.md section 6): spoke rows + hub tails (4 B per
+                # element), b_ij per hub-spoke pair, two bin bytes per hit (+ two fp64 weights when weighted)
+                pc.update(spoke=sp, tail=tl, edges=e, hits=t,
+                          bytes=4.0 * sp + 4.0 * tl + e + 2.0 * t)
+            per.append(pc)
             g.free()
-        return tri, st
+        return tri, st, per
 
     def timed(host: bool, steps: int, warmup: int):
         for _ in range(warmup):
@@ -206,35 +243,47 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-        total_ms, tri, agg = 0.0, 0, None
+        total_ms, tri, agg, per_agg = 0.0, 0, None, None
         for _ in range(steps):
             flush.fill_(1)                      # flush L2 between timed iterations (not timed)
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            tri, st = step(host)
+            tri, st, per = step(host)
             e1.record()
             torch.cuda.synchronize()
             total_ms += e0.elapsed_time(e1)
             agg = st if agg is None else {k: agg[k] + st[k] for k in st}
+            per_agg = [p["enum_ms"] for p in per] if per_agg is None else [a + p["enum_ms"] for a, p in zip(per_agg, per)]
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item()) / steps, tri, {k: v / steps for k, v in agg.items()}
+        return (max_over_ranks(total_ms, "cuda") / steps, tri, {k: v / steps for k, v in agg.items()},
+                [a / steps for a in per_agg])
 
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    _, work = step(False, count_work=True)          # untimed: exact work counters of this workload
-    ms, tri, st = timed(False, args.steps, args.warmup)
-    st["bytes"] = work["bytes"]
+    _, _, work = step(False, count_work=True)       # untimed: exact work counters of this workload
+    ms, tri, st, enum_ms = timed(False, args.steps, args.warmup)
     clocks = sampler.stop() if rank == 0 else None
-    ms_e2e, tri2, _ = timed(True, max(1, args.steps // 2), 1)
+    ms_e2e, tri2, _, _ = timed(True, max(1, args.steps // 2), 1)
     assert tri2 == tri
+    tri_all = sum_over_ranks(float(tri), "cuda")
+
+    # second headline of BASELINE.json's metric: 4pCF quadruplets/s on configs[2] (query only, rank 0, untimed region)
+    four = None
+    if rank == 0 and not args.no_4pcf:
+        c3 = cat.config3()
+        g = gr.gramsci_build_graph(torch.from_numpy(c3["points"]).cuda(), None, c3["box"], c3["r_min"], c3["r_max"], c3["nbins"])
+        best = None
+        for _ in range(3):
+            ec, _ = g.pcf4()
+            best = g.timing(1) if best is None else min(best, g.timing(1))
+        four = {"workload": "cfg3", "quadruplets": int(ec.sum()), "query_ms": best,
+                "quadruplets_per_s": float(ec.sum()) / (best * 1e-3)}
+        g.free()
 
     if rank != 0:
         if world > 1:
@@ -243,10 +292,14 @@ def run_ours(args):
     peak, peak_kind, peaks = load_peaks()
     h2d = sum(c["points"].nbytes + (0 if c["weights"] is None else c["weights"].nbytes) for c in cats)
     d2h = sum(8 * c["nbins"] ** 3 * (1 if c["weights"] is None else 2) for c in cats)
-    enum_s = st["enum_ms"] * 1e-3
-    achieved = st["bytes"] / enum_s / 1e9 if enum_s > 0 and st["bytes"] else None
+    # roofline of the dominant kernel = the enumeration launch with the largest share of the step
+    dom = max(range(len(cats)), key=lambda k: enum_ms[k])
+    dw = work[dom]
+    dom_s = enum_ms[dom] * 1e-3
+    achieved = dw["bytes"] / dom_s / 1e9
+    kern = ("k_3pcf_table" if args.algo != 2 else "k_3pcf_bsearch") + ("<weighted>" if dw["weighted"] else "<counts>")
     line = {
-        "metric": "3pCF triangles/s", "value": world * tri / (ms * 1e-3), "unit": "triangles/s",
+        "metric": "3pCF triangles/s", "value": tri_all / (ms * 1e-3), "unit": "triangles/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "catalogues": [c["name"] for c in cats],
@@ -255,17 +308,22 @@ def run_ours(args):
                    "step": "graph build + 3pCF + fold for every catalogue", "l2": "flushed between timed steps "
                    "(256 MiB write); CSR (>=0.3 GB per catalogue) exceeds the 126 MB L2",
                    "algo": args.algo, "build_ms": st["build_ms"], "query_ms": st["query_ms"],
-                   "enum_kernel_ms": st["enum_ms"], "query_only_triangles_per_s": tri / (st["query_ms"] * 1e-3)},
+                   "enum_kernel_ms": st["enum_ms"], "enum_kernel_ms_per_catalogue": enum_ms,
+                   "query_only_triangles_per_s": tri / (st["query_ms"] * 1e-3), "four_pcf": four},
         "clocks": clocks,
-        "e2e": {"value": world * tri / (ms_e2e * 1e-3), "unit": "triangles/s", "h2d_bytes_per_step": h2d,
+        "e2e": {"value": tri_all / (ms_e2e * 1e-3), "unit": "triangles/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
         "gpu_launches": int(round(st["launches"] * args.steps)),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": (achieved / peak) if achieved else None, "traffic": None,
-                     "kernel": "k_3pcf (enumeration)", "peak_kind": f"hbm copy, {peak_kind}",
-                     "algorithmic_bytes_per_step": st["bytes"],
-                     "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits "
-                             "(SURVEY 8(d)); spoke rows are re-read from L2, so achieved may exceed the HBM peak"},
+                     "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(kern),
+                     "kernel": f"{kern} on {dw['name']}", "peak_kind": f"hbm copy, {peak_kind}",
+                     "launch_ms": enum_ms[dom], "algorithmic_bytes_per_launch": dw["bytes"],
+                     "units_per_launch": {"spoke_row_elements": dw["spoke"], "tail_elements": dw["tail"],
+                                          "hub_spoke_pairs": dw["edges"], "hits": dw["hits"]},
+                     "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits (DESIGN.md "
+                             "section 6); spoke rows are re-read from L2/L1, so this is an L2->SM figure and may "
+                             "exceed the HBM peak; traffic = dram read+write of one ncu --set full launch "
+                             "(profiles/)"},
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(cats)
@@ -284,6 +342,7 @@ def main():
     ap.add_argument("--algo", type=int, default=0)
     ap.add_argument("--ref-stride", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-4pcf", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

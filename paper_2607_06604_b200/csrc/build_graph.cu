@@ -516,14 +516,27 @@ k_row_stats(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, in
     if (threadIdx.x < 2 * (GR_S_MAX - GR_S_MIN + 1) && s_max[threadIdx.x] > 0) atomicMax(&out[threadIdx.x], s_max[threadIdx.x]);
 }
 
-// largest neighbour label stored in edges [lo,hi) (which search windows a hub window reaches; tiler.cu)
-__global__ void k_max_label(const int32_t *__restrict__ idx, int64_t lo, int64_t hi, int32_t *__restrict__ out)
+// which search windows the edges [lo,hi) of a hub window reach: bit c of out[0..] is set iff some neighbour
+// label lies in window c (row boundaries wlo[0..W], W <= 1024); tiler.cu visits only those tiles
+__global__ void k_need_mask(const int32_t *__restrict__ idx, int64_t lo, int64_t hi, const int32_t *__restrict__ wlo,
+                            int W, unsigned int *__restrict__ out)
 {
-    int m = -1;
-    for (int64_t e = lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < hi; e += (int64_t)gridDim.x * blockDim.x)
-        m = max(m, idx[e]);
-    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m >= 0) atomicMax(out, m);
+    extern __shared__ unsigned int s_mask[];
+    for (int t = threadIdx.x; t < (W + 31) / 32; t += blockDim.x) s_mask[t] = 0;
+    __syncthreads();
+    for (int64_t e = lo + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < hi; e += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t k = idx[e];
+        int a = 0, b = W;                    // largest c with wlo[c] <= k
+        while (b - a > 1) {
+            const int mid = (a + b) >> 1;
+            if (wlo[mid] <= k) a = mid; else b = mid;
+        }
+        const unsigned bit = 1u << (a & 31);
+        if (!(s_mask[a >> 5] & bit)) atomicOr(&s_mask[a >> 5], bit);
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < (W + 31) / 32; t += blockDim.x)
+        if (s_mask[t]) atomicOr(&out[t], s_mask[t]);
 }
 
 inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64_t>(1, (n + per - 1) / per); }
@@ -763,8 +776,20 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         if (g->has_pix) wpix.alloc((size_t)maxlen);
         const int Wn = (int)g->windows.size();
         g->need.assign((size_t)Wn * Wn, 0);
-        DevBuf<int32_t> dmax;
-        dmax.alloc(1);
+        if (Wn > 1024) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small: %d windows", Wn);
+        const int mwords = (Wn + 31) / 32;
+        DevBuf<unsigned int> dmask;
+        DevBuf<int32_t> dwlo;
+        dmask.alloc((size_t)mwords);
+        dwlo.alloc((size_t)Wn + 1);
+        std::vector<unsigned int> hmask((size_t)mwords);
+        {
+            std::vector<int32_t> hw((size_t)Wn + 1);
+            for (int c = 0; c < Wn; ++c) hw[c] = g->windows[c].row_lo;
+            hw[Wn] = (int32_t)n;
+            GR_CUDA(cudaMemcpyAsync(dwlo.p, hw.data(), sizeof(int32_t) * (Wn + 1), cudaMemcpyHostToDevice, st));
+            GR_CUDA(cudaStreamSynchronize(st));
+        }
         int hwin = 0;
         for (auto &w : g->windows) {
             int64_t len = w.e_hi - w.e_lo;
@@ -781,15 +806,15 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
                                                                                            w.row_lo, w.row_hi, stats.p);
             launches += 1;
             int64_t head = hptr[w.row_lo] - w.e_lo;   // entries before the first row belong to the previous window
-            // search windows this hub window reaches: spokes have larger labels than their hub, so [hwin, window of the largest label]
-            int32_t hmax = -1;
-            GR_CUDA(cudaMemsetAsync(dmax.p, 0xff, sizeof(int32_t), st));
-            if (len > head) k_max_label<<<296, 256, 0, st>>>(widx.p, head, len, dmax.p);
-            GR_CUDA(cudaMemcpyAsync(&hmax, dmax.p, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+            // search windows this hub window reaches (exact)
+            GR_CUDA(cudaMemsetAsync(dmask.p, 0, sizeof(unsigned int) * mwords, st));
+            if (len > head)
+                k_need_mask<<<296, 256, sizeof(unsigned int) * mwords, st>>>(widx.p, head, len, dwlo.p, Wn, dmask.p);
+            GR_CUDA(cudaMemcpyAsync(hmask.data(), dmask.p, sizeof(unsigned int) * mwords, cudaMemcpyDeviceToHost, st));
             GR_CUDA(cudaStreamSynchronize(st));
             launches += 1;
-            for (int c = hwin; c < Wn; ++c)
-                if (hmax >= g->windows[c].row_lo) g->need[(size_t)hwin * Wn + c] = 1;
+            for (int c = 0; c < Wn; ++c)
+                if (hmask[c >> 5] & (1u << (c & 31))) g->need[(size_t)hwin * Wn + c] = 1;
             ++hwin;
             GR_CUDA(cudaMemcpyAsync(g->h_idx + w.e_lo + head, widx.p + head, (size_t)(len - head) * 4, cudaMemcpyDeviceToHost, st));
             GR_CUDA(cudaMemcpyAsync(g->h_bin + w.e_lo + head, wbin.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));

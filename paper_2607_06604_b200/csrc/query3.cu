@@ -158,11 +158,12 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
 // of x-adjacent cells), so the table is a few KB; sizes come from the row statistics of the build.
 // Set-up and tear-down touch only the row's own entries (O(len)).
 //
-// Work mapping: G warps share one hub (G = 1, 2, 4, 8 by table size); each warp takes blocks of 32 spokes
-// and walks the concatenation of their rows N+(j) as ONE flat index space ("every lane always has an
-// element": rows are tens of entries long in the 1e6-point configurations, so a per-row 32-lane loop would
-// idle a third of the lanes and serialise the ptr -> idx load latency per row).  The spoke a lane's element
-// belongs to is recovered from a start-bit mask of the rows beginning inside the 32-element window.
+// Work mapping: G warps share one hub (G = 1, 2, 4, 8 by table size); each warp takes blocks of 32 spokes:
+// the lanes fetch the 32 row heads (ptr[j], ptr[j+1]) at once, then the warp streams the rows N+(j) one
+// after the other, 32 elements per window, with the first two windows of the next row already in flight
+// (rows are tens of entries long in the 1e6-point configurations, so the ptr -> idx latency chain per row
+// is what has to be hidden).  An earlier variant walked the 32 rows as one flat index space (no idle lanes)
+// but paid ~57 instructions per window for the bookkeeping; this one needs ~25.
 template <int G>
 __device__ __forceinline__ void group_sync(int group)
 {
@@ -182,7 +183,7 @@ struct T3Params {
     int hub_batch;      // schedule slots fetched per atomic
 };
 
-template <bool WEIGHTED, int G>
+template <bool WEIGHTED, int G, int U>      // U = windows in flight per trip on long rows
 __global__ void __launch_bounds__(Q3_THREADS)
 k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
              unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
@@ -199,13 +200,11 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
     // (plain pointer arithmetic on `smem` only: a round trip through an integer would turn every access
     // below into a generic-address load instead of LDS)
     unsigned char *gs = smem + (((size_t)p.nh * 4 + 15) & ~(size_t)15) + (size_t)group * p.group_bytes;
-    // group: [a_w f64 row_cap (W)] [flat arrays per warp] [pt u16] [tab] [a_bin u8 row_cap (W)]
+    // group: [a_w f64 row_cap (W)] [row heads per warp] [pt u16] [tab] [a_bin u8 row_cap (W)]
     double *a_w = (double *)gs;
     unsigned char *q = gs + (WEIGHTED ? (size_t)p.row_cap * 8 : 0);
-    long long *s_base = (long long *)q + gw * 32;           q += (size_t)G * 32 * 8;
+    int4 *s_head = (int4 *)q + gw * 32;                      q += (size_t)G * 32 * 16;   // (row offset lo, hi, len, b_ij nb^2)
     double *s_wia = (double *)q + gw * 32;                  q += WEIGHTED ? (size_t)G * 32 * 8 : 0;
-    int *s_hb = (int *)q + gw * 32;                         q += (size_t)G * 32 * 4;
-    int *s_off = (int *)q + gw * 32;                        q += (size_t)G * 32 * 4;
     uint16_t *pt = (uint16_t *)q;                           q += ((size_t)p.pt_len * 2 + 15) & ~(size_t)15;
     slot_t *tab = (slot_t *)q;                              q += ((size_t)p.tab_len * sizeof(slot_t) + 15) & ~(size_t)15;
     uint8_t *a_bin = (uint8_t *)q;
@@ -331,7 +330,26 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
         group_sync<G>(group);
 
         const double wi = WEIGHTED ? v.w[i] : 1.0;
-        // ---- blocks of 32 spokes, rows walked as one flat index space ----
+        // ---- blocks of 32 spokes: lanes fetch the row heads (ptr[j], ptr[j+1]) of 32 spokes at once, then the
+        // warp walks the rows one after the other; the first two windows of the NEXT row are in flight while
+        // the current row is looked up (rows are tens of entries long in the 1e6-point configurations)
+        auto lookup = [&](int32_t k, unsigned gam, int hb, double wia) {
+            const bool hi = k >= brk;
+            const unsigned d = min((unsigned)(k - (hi ? sub_hi : base)), hi ? 0xffffffffu : guard);
+            const unsigned ch = pt[min(d >> sh, ptl1)];
+            const unsigned e = tab[(ch << sh) | (d & pm)];
+            if (e != EMPTY) {
+                if (WEIGHTED) {
+                    const int h = hb + (int)a_bin[e] * nb + (int)gam;
+                    if (p.want_counts) atomicAdd(&hist[h], 1u);
+                    atomicAdd(&my_w[h], wia * a_w[e]);
+                } else {
+                    atomicAdd(&hist[hb + (int)e * nb + (int)gam], 1u);
+                }
+            }
+        };
+        const int32_t dead = base - 1;                 // below the row: lands on the guard page, never a member
+        const int32_t last = gi[n - 1];
         for (int a0 = gw * 32; a0 < n - 1; a0 += G * 32) {
             const int a = a0 + lane;
             int nj = 0, hb = 0;
@@ -349,66 +367,56 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             const unsigned nz = __ballot_sync(0xffffffffu, nj > 0);
             const int m = __popc(nz);
             if (m == 0) continue;
-            int incl = nj;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += y;
-            }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
             __syncwarp();
             if (nj > 0) {
                 const int r = __popc(nz & lt_mask);
-                s_base[r] = (long long)(jb - v.e0_c) - (long long)(incl - nj);
-                s_hb[r] = hb;
-                s_off[r] = incl - nj;
+                s_head[r] = make_int4((int)((jb - v.e0_c) & 0xffffffffll), (int)((jb - v.e0_c) >> 32), nj, hb);
                 if (WEIGHTED) s_wia[r] = wia;
             }
             __syncwarp();
-            const int myoff = (lane < m) ? s_off[lane] : INT32_MAX;
-            budget += (unsigned long long)total;
-
-            int cum = 0;
-            // U windows of 32 elements per trip: all U index loads are issued before the first look-up
-            constexpr int U = 4;
-            for (int f0 = 0; f0 < total; f0 += 32 * U) {
-                int32_t kk[U];
-                unsigned gam[U];
-                int sp[U];
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int fu = f0 + 32 * u;
-                    kk[u] = base - 1;                      // below the row: lands on the guard page, never a member
-                    gam[u] = 0;
-                    sp[u] = 0;
-                    if (fu < total) {
-                        const int rel = myoff - fu;
-                        const unsigned sm = __reduce_or_sync(0xffffffffu, (rel >= 0 && rel < 32) ? (1u << rel) : 0u);
-                        sp[u] = cum + __popc(sm & le_mask) - 1;
-                        cum += __popc(sm);
-                        if (fu + lane < total) {
-                            const long long ad = s_base[sp[u]] + fu + lane;
-                            kk[u] = v.idx_c[ad];
-                            gam[u] = v.bin_c[ad];
-                        }
-                    }
+            // prologue: first two windows of row 0
+            int4 hd = s_head[0];
+            double w_cur = WEIGHTED ? s_wia[0] : 0.0;
+            const int32_t *pi = v.idx_c + (((long long)hd.y << 32) | (unsigned)hd.x) + lane;
+            const uint8_t *pb = v.bin_c + (((long long)hd.y << 32) | (unsigned)hd.x) + lane;
+            int32_t k0 = dead, k1 = dead;
+            unsigned g0 = 0, g1 = 0;
+            if (lane < hd.z) { k0 = pi[0]; g0 = pb[0]; }
+            if (lane + 32 < hd.z) { k1 = pi[32]; g1 = pb[32]; }
+            for (int q = 0; q < m; ++q) {
+                const int njc = hd.z, hbc = hd.w;
+                const double wc = w_cur;
+                const int32_t *pic = pi;
+                const uint8_t *pbc = pb;
+                const int32_t c0 = k0, c1 = k1;
+                const unsigned e0g = g0, e1g = g1;
+                if (q + 1 < m) {                               // next row's first two windows
+                    hd = s_head[q + 1];
+                    if (WEIGHTED) w_cur = s_wia[q + 1];
+                    pi = v.idx_c + (((long long)hd.y << 32) | (unsigned)hd.x) + lane;
+                    pb = v.bin_c + (((long long)hd.y << 32) | (unsigned)hd.x) + lane;
+                    k0 = dead; k1 = dead;
+                    if (lane < hd.z) { k0 = pi[0]; g0 = pb[0]; }
+                    if (lane + 32 < hd.z) { k1 = pi[32]; g1 = pb[32]; }
                 }
+                budget += (unsigned long long)njc;
+                lookup(c0, e0g, hbc, wc);
+                // rows are sorted: once a window starts beyond the hub's last neighbour nothing further can hit
+                if (njc > 32 && __shfl_sync(0xffffffffu, c1, 0) <= last) lookup(c1, e1g, hbc, wc);
+                if (njc > 64 && __shfl_sync(0xffffffffu, c1, 31) > last) continue;
+                for (int t0 = 64; t0 < njc; t0 += 32 * U) {
+                    int32_t kk[U];
+                    unsigned gg[U];
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int32_t k = kk[u];
-                    const bool hi = k >= brk;
-                    const unsigned d = min((unsigned)(k - (hi ? sub_hi : base)), hi ? 0xffffffffu : guard);
-                    const unsigned ch = pt[min(d >> sh, ptl1)];
-                    const unsigned e = tab[(ch << sh) | (d & pm)];
-                    if (e != EMPTY) {
-                        if (WEIGHTED) {
-                            const int h = s_hb[sp[u]] + (int)a_bin[e] * nb + (int)gam[u];
-                            if (p.want_counts) atomicAdd(&hist[h], 1u);
-                            atomicAdd(&my_w[h], s_wia[sp[u]] * a_w[e]);
-                        } else {
-                            atomicAdd(&hist[s_hb[sp[u]] + (int)e * nb + (int)gam[u]], 1u);
-                        }
+                    for (int u = 0; u < U; ++u) {
+                        kk[u] = dead;
+                        gg[u] = 0;
+                        if (t0 + 32 * u + lane < njc) { kk[u] = pic[t0 + 32 * u]; gg[u] = pbc[t0 + 32 * u]; }
                     }
+#pragma unroll
+                    for (int u = 0; u < U; ++u)
+                        if (t0 + 32 * u < njc) lookup(kk[u], gg[u], hbc, wc);
+                    if (__shfl_sync(0xffffffffu, kk[U - 1], 31) > last) break;     // (a dead lane 31 = end of the row anyway)
                 }
             }
             // uint32 bins cannot wrap: any bin holds at most the hits all 8 warps added since their own last
@@ -511,28 +519,28 @@ struct Q3Run {
     double *raw_w;
     int grid;
     size_t smem;
-    int use_table, G;
+    int use_table, G, long_rows;
 };
 
-template <bool W>
+template <bool W, int U>
 void launch_table(const Q3Run *r, const GrView &v, cudaStream_t st)
 {
     switch (r->G) {
-        case 1: k_3pcf_table<W, 1><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
-        case 2: k_3pcf_table<W, 2><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
-        case 4: k_3pcf_table<W, 4><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
-        default: k_3pcf_table<W, 8><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        case 1: k_3pcf_table<W, 1, U><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        case 2: k_3pcf_table<W, 2, U><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        case 4: k_3pcf_table<W, 4, U><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
+        default: k_3pcf_table<W, 8, U><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->t, r->counter, r->raw_cnt, r->raw_w); break;
     }
 }
 
-template <bool W>
+template <bool W, int U>
 const void *table_fn(int G)
 {
     switch (G) {
-        case 1: return (const void *)k_3pcf_table<W, 1>;
-        case 2: return (const void *)k_3pcf_table<W, 2>;
-        case 4: return (const void *)k_3pcf_table<W, 4>;
-        default: return (const void *)k_3pcf_table<W, 8>;
+        case 1: return (const void *)k_3pcf_table<W, 1, U>;
+        case 2: return (const void *)k_3pcf_table<W, 2, U>;
+        case 4: return (const void *)k_3pcf_table<W, 4, U>;
+        default: return (const void *)k_3pcf_table<W, 8, U>;
     }
 }
 
@@ -541,8 +549,8 @@ void tile_3pcf(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
     Q3Run *r = (Q3Run *)user;
     GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
     if (r->use_table) {
-        if (r->p.weighted) launch_table<true>(r, v, st);
-        else launch_table<false>(r, v, st);
+        if (r->p.weighted) { if (r->long_rows) launch_table<true, 8>(r, v, st); else launch_table<true, 4>(r, v, st); }
+        else { if (r->long_rows) launch_table<false, 8>(r, v, st); else launch_table<false, 4>(r, v, st); }
     } else if (r->p.weighted)
         k_3pcf_bsearch<true><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
     else
@@ -560,7 +568,7 @@ size_t table_group_bytes(const gramsci_graph *g, int s, bool weighted, int G, in
     if (ptl > (1 << 20) || tbl > (1 << 20) || g->max_pages[s] >= 65535) return 0;
     *pt_len = (int)ptl;
     *tab_len = (int)tbl;
-    size_t b = (size_t)G * 32 * (8 + 4 + 4 + (weighted ? 8 : 0));
+    size_t b = (size_t)G * 32 * (16 + (weighted ? 8 : 0));
     b += ((size_t)ptl * 2 + a16) & ~a16;
     b += ((size_t)tbl * (weighted ? 2 : 1) + a16) & ~a16;
     if (weighted) b += (size_t)row_cap * 8 + (((size_t)row_cap + a16) & ~a16);
@@ -611,6 +619,8 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     // ---- slot-table kernel: page shift s minimising the table, then the smallest group that fits ----
     r.use_table = 0;
     r.G = 8;
+    // rows of hundreds of entries and more stream from DRAM (the CSR no longer lives in L2): keep 8 windows in flight
+    r.long_rows = (g->n > 0 && g->n_edges / g->n >= 512) ? 1 : 0;
     if (g->algo != GRAMSCI_ALGO_BSEARCH && g->max_row >= 2 && g->max_row < 65535) {
         const size_t hist_bytes = (((size_t)nh * 4 + 15) & ~(size_t)15) + 16;
         int best_s = -1, ptl = 0, tbl = 0;
@@ -644,7 +654,8 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     }
     const void *fn;
     if (r.use_table) {
-        fn = W ? table_fn<true>(r.G) : table_fn<false>(r.G);
+        fn = W ? (r.long_rows ? table_fn<true, 8>(r.G) : table_fn<true, 4>(r.G))
+               : (r.long_rows ? table_fn<false, 8>(r.G) : table_fn<false, 4>(r.G));
     } else {
         r.p.smem_hist = ((size_t)nh * 4 <= 96 * 1024) ? 1 : 0;
         size_t per_entry = 4 + 1 + (W ? 8 : 0);

@@ -1,0 +1,57 @@
+"""The N > 1 host logic of bench.py on CPU: two gloo ranks shard the workload by seed (independent
+catalogues, no data-path collective), the step time is the max over ranks and the job total the sum.
+The per-rank "device time" here is faked (there is no GPU in this test); what is checked is the
+sharding rule and the reductions bench.py applies to the numbers it prints."""
+import os
+import socket
+import sys
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank: int, world: int, port: int, out_dir: str):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import bench
+    import catalogues as cat
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cats = bench.workload("cfg1", seed_shift=bench.rank_seed_shift(rank))
+    pts = cats[0]["points"]
+    fake_ms = 10.0 + 5.0 * rank                   # rank 1 is the slow one
+    fake_units = float(pts.shape[0] + rank)
+    t = bench.max_over_ranks(fake_ms)
+    u = bench.sum_over_ranks(fake_units)
+    dist.barrier()
+    np.save(os.path.join(out_dir, f"r{rank}.npy"), np.array([t, u, pts[0, 0], float(len(cats))]))
+    dist.destroy_process_group()
+
+
+def test_two_rank_sharding_and_reductions(tmp_path):
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    r0 = np.load(tmp_path / "r0.npy")
+    r1 = np.load(tmp_path / "r1.npy")
+    assert r0[0] == r1[0] == 15.0                 # max over ranks, identical on every rank
+    assert r0[1] == r1[1] == 2000 + 2001          # whole-job units = sum over ranks
+    assert r0[2] != r1[2]                         # different seeds -> different catalogues per rank
+    assert r0[3] == r1[3] == 1.0
+
+
+def test_single_process_reductions_are_identity():
+    import bench
+    assert bench.max_over_ranks(3.5) == 3.5
+    assert bench.sum_over_ranks(7.0) == 7.0
+    assert bench.rank_seed_shift(0) == 0 and bench.rank_seed_shift(3) != bench.rank_seed_shift(2)
