@@ -9,18 +9,21 @@
 //   phase 1 (per hub i, = the 3pCF membership pass): row a of the local matrix D is
 //            D[a][p] = bin of edge (k_a, k_p) if k_p in N+(k_a) else 0xFF,   a < p < n = len(N+(i)),
 //            found by one lane-parallel search of every element of N+(k_a) in the staged hub row;
-//   phase 2: for every local edge (a,b) (D[a][b] != 0xFF) a warp streams rows a and b of D with
-//            coalesced 4-byte loads; every c > b with D[a][c] and D[b][c] both set is a 4-clique
-//            i < k_a < k_b < k_c, found exactly once (oriented storage, A-1, A-15), and is histogrammed by
-//            its raw 6-tuple (b_ia, b_ib, b_ic, b_ab, b_ac, b_bc) = the order (b12,b13,b14,b23,b24,b34).
+//   phase 2: D also exists as bit rows.  Warps scan the bit rows for local edges (a,b), compact them with
+//            ballots into a small queue, and every LANE takes one local edge: the set bits c > b of
+//            bits[a] & bits[b] are the 4-cliques i < k_a < k_b < k_c, each found exactly once (oriented
+//            storage, A-1, A-15) and histogrammed by its raw 6-tuple (b_ia, b_ib, b_ic, b_ab, b_ac, b_bc)
+//            = the order (b12,b13,b14,b23,b24,b34).  (A first version gave a warp to each local edge and
+//            streamed the byte rows; with rows of ~50 entries most lanes idled: 37 ms vs now on cfg3.)
 //
 // Parity (Eq. 3; A-8..A-11): V = (n_a x n_b) . n_c on the pixel-centre unit vectors of the three
 // hub spokes, every product and sum rounded separately; the kernel accumulates sign(V) (0 when
 // |V| < 1e-9) per RAW tuple and the fold applies the chirality factor of the raw tuple, which for the
 // raw tuple t^sigma of a canonical chiral tuple t is sgn(sigma) (and 0 for bin-achiral t).
 //
-// D lives in a per-CTA slice of a global scratch (the paper's "per-gang slice of a global scratch sized
-// from the longest row"); it is written and read by the same CTA only and stays in L1/L2.
+// D lives in shared memory when the longest row allows (a few hundred entries), else in a per-CTA slice of a
+// global scratch (the paper's "per-gang slice of a global scratch sized from the longest row"),
+// written and read by the same CTA only (L1/L2 resident).
 // Raw histograms are nb^6 bins -- too large for shared memory (8^6 x 4 B = 1 MiB) -- so hits go to
 // global memory with RED atomics, spread over a few shards that the fold sums.
 #include "internal.cuh"
@@ -57,24 +60,39 @@ __device__ __forceinline__ int lower_bound_s(const int32_t *a, int lo, int hi, i
 
 // ---- enumeration ---------------------------------------------------------------------------------------
 // cnt_e/cnt_o/w_e/w_o: [n_shards][nh] raw histograms (any may be null).
+// SMALL: the local matrix D (bytes) and its bit rows live in shared memory (rows up to a few hundred
+// entries); otherwise in the CTA's slice of the global scratch.
+template <bool SMALL>
 __global__ void __launch_bounds__(Q4_THREADS)
 k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *scratch, size_t scratch_stride,
        const double *__restrict__ pix_tab, unsigned long long *__restrict__ cnt_e,
        unsigned long long *__restrict__ cnt_o, double *__restrict__ w_e, double *__restrict__ w_o)
 {
     extern __shared__ __align__(16) unsigned char smem[];
-    // layout: [tab 256*3*8 (parity)] [w row_cap*8 (weighted)] [idx row_cap*4] [t3 row_cap*4] [pix row_cap]
+    // layout: [tab 256*3*8 (parity)] [w row_cap*8 (weighted)] [idx row_cap*4] [t3 row_cap*4] [queues 8*64*4]
+    //         [pix row_cap] [SMALL: D row_cap*row_cap, bits row_cap*(row_cap/32)*4]
     double *s_tab = (double *)smem;
     double *a_w = (double *)(smem + (p.parity ? 256 * 3 * 8 : 0));
     int32_t *a_idx = (int32_t *)((unsigned char *)a_w + (p.weighted ? (size_t)p.row_cap * 8 : 0));
     uint32_t *a_t3 = (uint32_t *)(a_idx + p.row_cap);       // b_ic * nb^3
-    uint8_t *a_pix = (uint8_t *)(a_t3 + p.row_cap);
+    uint32_t *s_queue = a_t3 + p.row_cap;                   // per warp: 64 pending local edges (a << 16 | b)
+    uint8_t *a_pix = (uint8_t *)(s_queue + Q4_WARPS * 64);
     __shared__ int s_slot;
 
     const int nb = p.nb;
     const uint32_t nb2 = nb * nb, nb3 = nb2 * nb;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    uint8_t *D = scratch + (size_t)blockIdx.x * scratch_stride;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    uint8_t *D;
+    uint32_t *bits;
+    if (SMALL) {
+        D = a_pix + p.row_cap;
+        bits = (uint32_t *)(D + (size_t)p.row_cap * p.row_cap);
+    } else {
+        D = scratch + (size_t)blockIdx.x * scratch_stride;
+        bits = (uint32_t *)(D + (size_t)p.row_cap * p.row_cap);
+    }
+    uint32_t *my_q = s_queue + warp * 64;
     const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh;
     if (cnt_e) cnt_e += shard;
     if (cnt_o) cnt_o += shard;
@@ -93,7 +111,8 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         const int64_t rb = v.ptr[i], re = v.ptr[i + 1];
         const int n = (int)(re - rb);
         if (n < 3) continue;                                   // a 4-clique needs three spokes
-        const int ld = (n + 15) & ~15;                         // row stride of D
+        const int ld = (n + 15) & ~15;                         // row stride of D (bytes)
+        const int nw = (n + 31) >> 5;                          // row stride of bits (words)
         const int32_t *gi = v.idx_h + (rb - v.e0_h);
         const uint8_t *gb = v.bin_h + (rb - v.e0_h);
         const uint8_t *gp = v.pix_h ? v.pix_h + (rb - v.e0_h) : nullptr;
@@ -104,16 +123,16 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
             if (p.parity) a_pix[t] = gp[t];
             if (p.weighted) a_w[t] = v.w[k];
         }
-        // D := 0xFF
-        {
-            uint4 ff = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+        {   // D := 0xFF, bits := 0
+            const uint4 ff = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
             uint4 *D4 = (uint4 *)D;
             const int total = (n * ld) >> 4;
             for (int t = threadIdx.x; t < total; t += Q4_THREADS) D4[t] = ff;
+            for (int t = threadIdx.x; t < n * nw; t += Q4_THREADS) bits[t] = 0u;
         }
         __syncthreads();
 
-        // ---- phase 1: local connectivity matrix ----
+        // ---- phase 1: local connectivity matrix (bytes) and its bit rows ----
         for (int a = warp; a < n - 1; a += Q4_WARPS) {
             const int32_t j = a_idx[a];
             const int64_t jb = v.ptr[j], je = v.ptr[j + 1];
@@ -122,70 +141,88 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
             const uint8_t *Bb = v.bin_c + (jb - v.e0_c);
             const int32_t t_last = a_idx[n - 1];
             uint8_t *Da = D + (size_t)a * ld;
+            uint32_t *Ba = bits + (size_t)a * nw;
             int lo = a + 1;
             for (int t0 = 0; t0 < nj; t0 += 32) {
                 const int t = t0 + lane;
                 const int32_t k = (t < nj) ? B[t] : INT32_MAX;
                 int pos = n;
                 if (k <= t_last) pos = lower_bound_s(a_idx, lo, n, k);
-                if (pos < n && a_idx[pos] == k) Da[pos] = Bb[t];
+                if (pos < n && a_idx[pos] == k) {
+                    Da[pos] = Bb[t];
+                    atomicOr(&Ba[pos >> 5], 1u << (pos & 31));
+                }
                 lo = __shfl_sync(0xffffffffu, pos, 0);
                 if (__shfl_sync(0xffffffffu, k, 31) > t_last) break;
             }
         }
         __syncthreads();
 
-        // ---- phase 2: triangles of the local graph = 4-cliques under hub i ----
+        // ---- phase 2: triangles of the local graph = 4-cliques under hub i; one LANE per local edge (a,b) ----
         const double wi = p.weighted ? v.w[i] : 1.0;
-        for (int a = 0; a < n - 2; ++a) {
-            const uint8_t *Da = D + (size_t)a * ld;
-            const uint32_t base_a = (a_t3[a] / nb3) * (nb3 * nb2);             // b_ia * nb^5
-            double na0 = 0, na1 = 0, na2 = 0;
-            if (p.parity) { const double *q = s_tab + 3 * a_pix[a]; na0 = q[0]; na1 = q[1]; na2 = q[2]; }
-            const double wia = p.weighted ? wi * a_w[a] : 1.0;
-            for (int b = a + 1 + warp; b < n - 1; b += Q4_WARPS) {
-                const uint32_t g_ab = Da[b];
-                if (g_ab == 0xffu) continue;
-                const uint8_t *Db = D + (size_t)b * ld;
-                const uint32_t base = base_a + (a_t3[b] / nb3) * (nb3 * nb) + g_ab * nb2;   // + b_ib nb^4 + b_ab nb^2
-                double cx = 0, cy = 0, cz = 0;
-                if (p.parity) {
-                    const double *q = s_tab + 3 * a_pix[b];
-                    const double nb0 = q[0], nb1 = q[1], nb2d = q[2];
-                    cx = __dsub_rn(__dmul_rn(na1, nb2d), __dmul_rn(na2, nb1));
-                    cy = __dsub_rn(__dmul_rn(na2, nb0), __dmul_rn(na0, nb2d));
-                    cz = __dsub_rn(__dmul_rn(na0, nb1), __dmul_rn(na1, nb0));
-                }
-                const double wiab = p.weighted ? wia * a_w[b] : 1.0;
-                for (int c0 = ((b + 1) & ~3) + 4 * lane; c0 < n; c0 += 128) {
-                    const uint32_t ra = *(const uint32_t *)(Da + c0);
-                    const uint32_t rbw = *(const uint32_t *)(Db + c0);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const int c = c0 + q;
-                        const uint32_t g_ac = (ra >> (8 * q)) & 0xffu, g_bc = (rbw >> (8 * q)) & 0xffu;
-                        if (c > b && c < n && g_ac != 0xffu && g_bc != 0xffu) {
-                            const uint32_t x = base + a_t3[c] + g_ac * nb + g_bc;
-                            if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
-                            double ww = 0.0;
-                            if (p.weighted) {
-                                ww = wiab * a_w[c];
-                                atomicAdd(&w_e[x], ww);
-                            }
-                            if (p.parity) {
-                                const double *nc = s_tab + 3 * a_pix[c];
-                                const double V = __dadd_rn(__dadd_rn(__dmul_rn(cx, nc[0]), __dmul_rn(cy, nc[1])),
-                                                           __dmul_rn(cz, nc[2]));
-                                if (fabs(V) >= 1e-9) {
-                                    const bool pos = V > 0.0;
-                                    if (cnt_o) atomicAdd(&cnt_o[x], pos ? 1ull : ~0ull);     // += +-1 (mod 2^64)
-                                    if (w_o) atomicAdd(&w_o[x], pos ? ww : -ww);
-                                }
-                            }
+        auto process = [&](uint32_t pair) {
+            const int a = (int)(pair >> 16), b = (int)(pair & 0xffffu);
+            const uint8_t *Da = D + (size_t)a * ld, *Db = D + (size_t)b * ld;
+            const uint32_t *Ba = bits + (size_t)a * nw, *Bb2 = bits + (size_t)b * nw;
+            const uint32_t base = a_t3[a] * nb2 + a_t3[b] * nb + (uint32_t)Da[b] * nb2;   // b_ia nb^5 + b_ib nb^4 + b_ab nb^2
+            double cx = 0, cy = 0, cz = 0, wiab = 1.0;
+            if (p.parity) {
+                const double *qa = s_tab + 3 * a_pix[a], *qb = s_tab + 3 * a_pix[b];
+                cx = __dsub_rn(__dmul_rn(qa[1], qb[2]), __dmul_rn(qa[2], qb[1]));
+                cy = __dsub_rn(__dmul_rn(qa[2], qb[0]), __dmul_rn(qa[0], qb[2]));
+                cz = __dsub_rn(__dmul_rn(qa[0], qb[1]), __dmul_rn(qa[1], qb[0]));
+            }
+            if (p.weighted) wiab = wi * a_w[a] * a_w[b];
+            for (int w = (b + 1) >> 5; w < nw; ++w) {
+                uint32_t common = Ba[w] & Bb2[w];
+                if (w == ((b + 1) >> 5)) common &= ~((1u << ((b + 1) & 31)) - 1u);     // only c > b
+                while (common) {
+                    const int c = (w << 5) + __ffs(common) - 1;
+                    common &= common - 1u;
+                    const uint32_t x = base + a_t3[c] + (uint32_t)Da[c] * nb + (uint32_t)Db[c];
+                    if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
+                    double ww = 0.0;
+                    if (p.weighted) {
+                        ww = wiab * a_w[c];
+                        atomicAdd(&w_e[x], ww);
+                    }
+                    if (p.parity) {
+                        const double *nc = s_tab + 3 * a_pix[c];
+                        const double V = __dadd_rn(__dadd_rn(__dmul_rn(cx, nc[0]), __dmul_rn(cy, nc[1])),
+                                                   __dmul_rn(cz, nc[2]));
+                        if (fabs(V) >= 1e-9) {
+                            const bool pos = V > 0.0;
+                            if (cnt_o) atomicAdd(&cnt_o[x], pos ? 1ull : ~0ull);     // += +-1 (mod 2^64)
+                            if (w_o) atomicAdd(&w_o[x], pos ? ww : -ww);
                         }
                     }
                 }
             }
+        };
+        int qn = 0;                                            // warp-uniform queue fill
+        for (int a = warp; a < n - 2; a += Q4_WARPS) {
+            const uint32_t *Ba = bits + (size_t)a * nw;
+            for (int w = (a + 1) >> 5; w < nw; ++w) {          // lanes scan the 32 candidates b of word w
+                const int bcand = (w << 5) + lane;
+                const bool edge = bcand > a && bcand < n - 1 && ((Ba[w] >> lane) & 1u);
+                const unsigned m = __ballot_sync(0xffffffffu, edge);
+                if (edge) my_q[qn + __popc(m & lt_mask)] = ((uint32_t)a << 16) | (uint32_t)bcand;
+                qn += __popc(m);
+                __syncwarp();
+                if (qn >= 32) {
+                    const uint32_t pr = my_q[lane];
+                    const uint32_t rest = my_q[32 + lane];
+                    __syncwarp();
+                    my_q[lane] = rest;
+                    qn -= 32;
+                    process(pr);
+                    __syncwarp();
+                }
+            }
+        }
+        if (qn > 0) {
+            __syncwarp();
+            if (lane < qn) process(my_q[lane]);
         }
     }
 }
@@ -275,22 +312,29 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     if (channels == 0) { GR_CUDA(cudaStreamSynchronize(st)); g->t_query_ms = total.stop(); return; }
     p.n_shards = (int)std::max<int64_t>(1, std::min<int64_t>(8, ((int64_t)64 << 20) / (nh * 8 * channels)));
 
-    size_t smem = (p.parity ? 256 * 3 * 8 : 0) + (size_t)p.row_cap * (4 + 4 + 1 + (p.weighted ? 8 : 0)) + 64;
+    const size_t rc = (size_t)p.row_cap;
+    if (rc >= 65536) GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) exceeds 65535", g->max_row);
+    const size_t mat_bytes = rc * rc + rc * ((rc + 31) / 32) * 4;        // D (bytes) + bit rows
+    size_t smem = (p.parity ? 256 * 3 * 8 : 0) + rc * (4 + 4 + 1 + (p.weighted ? 8 : 0)) + Q4_WARPS * 64 * 4 + 64;
+    smem = (smem + 15) & ~(size_t)15;
+    const bool small = smem + mat_bytes <= 96 * 1024;
+    if (small) smem += mat_bytes;
     if (smem > g->smem_optin)
         GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
-    GR_CUDA(cudaFuncSetAttribute(k_4pcf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const void *fn = small ? (const void *)k_4pcf<true> : (const void *)k_4pcf<false>;
+    GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
-    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_4pcf, Q4_THREADS, smem));
+    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, Q4_THREADS, smem));
     occ = std::max(1, std::min(occ, 4));
     const int grid = g->sm_count * occ;
-    const size_t stride = (size_t)p.row_cap * p.row_cap;
+    const size_t stride = small ? 0 : ((mat_bytes + 255) & ~(size_t)255);
 
     DevBuf<uint8_t> scratch;
     DevBuf<unsigned int> counter;
     DevBuf<double> tab;
     DevBuf<unsigned long long> ce, co;
     DevBuf<double> we, wo;
-    scratch.alloc(stride * grid);
+    scratch.alloc(stride * grid + 256);
     counter.alloc(1);
     GR_CUDA(cudaMemsetAsync(counter.p, 0, sizeof(unsigned int), st));
     const size_t tot = (size_t)nh * p.n_shards;
@@ -325,8 +369,12 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     {
         GrTimer en(st);
         if (g->n > 0) {
-            k_4pcf<<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
-                                                   (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
+            if (small)
+                k_4pcf<true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
+                                                             (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
+            else
+                k_4pcf<false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
+                                                              (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
             GR_CUDA(cudaGetLastError());
             g->n_launches += 1;
         }
