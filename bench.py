@@ -16,6 +16,7 @@ different seed, no data-path collective ("weak" scaling); time = max over ranks.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -35,6 +36,9 @@ import catalogues as cat  # noqa: E402
 # ncu --set full capture (profiles/r1_b_table_3pcf_full.md)
 DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 578.146816e6 + 6.029568e6,
                       "k_3pcf_table<counts>": 301.713408e6 + 4.563456e6}
+
+
+RED_PEAK_GOPS = 186.0      # global RED.E.ADD.(U64|F64), spread addresses, all SMs (measured, see above)
 
 
 def load_peaks():
@@ -126,6 +130,14 @@ def workload(name: str, seed_shift: int = 0):
         return [cat.config1(seed=1001 + seed_shift)]
     if name == "cfg5p":       # scaled replica of configs[4] (same density, L=425)
         return [cat.config5(seed=5001 + seed_shift, n=39_062, L=425.0)]
+    if name == "cfg5":        # configs[4] in full: 2.5e6 points, 8.4e9 edges, 42 GB of CSR (use --steps 1 --warmup 0)
+        return [cat.config5(seed=5001 + seed_shift)]
+    if name == "cfg3":        # configs[2]: 4pCF (+ the 2pCF of the same graph for the disconnected term)
+        return [cat.config3(seed=3001 + seed_shift)]
+    if name == "cfg4":        # configs[3]: parity-decomposed 4pCF, weighted
+        return [cat.config4(seed=4001 + seed_shift)]
+    if name == "cfg4s":       # 1/8 replica of configs[3] (same density, 15 x 15 degree cap)
+        return [cat.config4(seed=4001 + seed_shift, n=62_500, cap_deg=15.0)]
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -213,12 +225,22 @@ def run_ours(args):
         tri = 0
         st = {"enum_ms": 0.0, "build_ms": 0.0, "query_ms": 0.0, "launches": 0.0, "edges": 0}
         per = []
+        digest = hashlib.sha1()
         for c, d, p in zip(cats, dev, pin):
             pts, w = (p if host else d)
-            g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo)
+            kind = c["kind"]
+            g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo,
+                                       want_pixels=(kind == "4pcf_parity"),
+                                       device_mem_cap_bytes=int(args.cap_gib * 2 ** 30))
             st["build_ms"] += g.timing(0)
             st["launches"] += g.timing(3)
-            cnt, ws = g.pcf3(counts=True, weighted=(w is not None), host=host)
+            if kind == "3pcf":
+                cnt, ws = g.pcf3(counts=True, weighted=(w is not None), host=host)
+            elif kind == "4pcf":
+                cnt, ws = g.pcf4(counts=True, weighted=(w is not None), host=host)
+            else:
+                cnt, _, ws, _ = g.pcf4_parity(counts=True, weighted=(w is not None), host=host)
+            digest.update(np.ascontiguousarray(cnt).tobytes())
             pc = {"name": c["name"], "enum_ms": g.timing(2), "weighted": w is not None}
             st["enum_ms"] += g.timing(2)
             st["query_ms"] += g.timing(1)
@@ -228,13 +250,18 @@ def run_ours(args):
             e = g.info()["n_edges"]
             st["edges"] += e
             if count_work:
-                sp, tl = g.work_counters()
+                sp, tl = g.work_counters() if kind == "3pcf" else (0, 0)
                 # algorithmic bytes of the enumeration: spoke rows + hub tails (4 B per
                 # element), b_ij per hub-spoke pair, two bin bytes per hit (+ two fp64 weights when weighted)
                 pc.update(spoke=sp, tail=tl, edges=e, hits=t,
                           bytes=4.0 * sp + 4.0 * tl + e + 2.0 * t)
+            pc["n_windows"] = g.info()["n_windows"]
+            pc["staged_bytes"] = g.timing(4)
             per.append(pc)
             g.free()
+        stats["sha1"] = digest.hexdigest()
+        stats["windows"] = [p_["n_windows"] for p_ in per]
+        stats["staged_bytes"] = sum(p_["staged_bytes"] for p_ in per)
         return tri, st, per
 
     def timed(host: bool, steps: int, warmup: int):
@@ -268,8 +295,11 @@ def run_ours(args):
     _, _, work = step(False, count_work=True)       # untimed: exact work counters of this workload
     ms, tri, st, enum_ms = timed(False, args.steps, args.warmup)
     clocks = sampler.stop() if rank == 0 else None
-    ms_e2e, tri2, _, _ = timed(True, max(1, args.steps // 2), 1)
-    assert tri2 == tri
+    if args.skip_e2e:
+        ms_e2e = None
+    else:
+        ms_e2e, tri2, _, _ = timed(True, max(1, args.steps // 2), 1)
+        assert tri2 == tri
     tri_all = sum_over_ranks(float(tri), "cuda")
 
     # second headline of BASELINE.json's metric: 4pCF quadruplets/s on configs[2] (query only, rank 0, untimed region)
@@ -297,33 +327,53 @@ def run_ours(args):
     dw = work[dom]
     dom_s = enum_ms[dom] * 1e-3
     achieved = dw["bytes"] / dom_s / 1e9
-    kern = ("k_3pcf_table" if args.algo != 2 else "k_3pcf_bsearch") + ("<weighted>" if dw["weighted"] else "<counts>")
+    kind0 = cats[0]["kind"]
+    unit = "triangles/s" if kind0 == "3pcf" else "quadruplets/s"
+    metric = "3pCF triangles/s" if kind0 == "3pcf" else ("4pCF quadruplets/s" if kind0 == "4pcf" else "parity-4pCF quadruplets/s")
+    if kind0 == "3pcf":
+        kern = ("k_3pcf_table" if args.algo != 2 else "k_3pcf_bsearch") + ("<weighted>" if dw["weighted"] else "<counts>")
+    else:
+        kern = "k_4pcf"
+    if kind0 == "3pcf":
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(kern) if args.workload == "cfg2" else None,
+                "kernel": f"{kern} on {dw['name']}", "peak_kind": f"hbm copy, {peak_kind}",
+                "launch_ms": enum_ms[dom], "algorithmic_bytes_per_launch": dw["bytes"],
+                "units_per_launch": {"spoke_row_elements": dw["spoke"], "tail_elements": dw["tail"],
+                                     "hub_spoke_pairs": dw["edges"], "hits": dw["hits"]},
+                "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits (DESIGN.md "
+                        "section 6); spoke rows are re-read from L2/L1, so this is an L2->SM figure and may "
+                        "exceed the HBM peak; traffic = dram read+write of one ncu --set full launch "
+                        "(profiles/)"}
+    else:
+        # 4pCF kernels are bound by the L2 atomic rate: one RED per hit and output channel;
+        # peak = RED.E.ADD.64 rate measured on this pool's B200 by csrc/ubench_atomics.cu (profiles/r1_ubench_atomics.txt)
+        ch = 1 if cats[dom]["weights"] is None else (4 if kind0 == "4pcf_parity" else 2)
+        red_rate = dw["hits"] * ch / dom_s / 1e9
+        roof = {"bound": "l2-atomics", "achieved": red_rate, "peak": RED_PEAK_GOPS, "unit": "Gatomic/s",
+                "frac": red_rate / RED_PEAK_GOPS, "traffic": None, "kernel": f"{kern} on {dw['name']}",
+                "launch_ms": enum_ms[dom], "units_per_launch": {"hits": dw["hits"], "channels": ch}}
     line = {
-        "metric": "3pCF triangles/s", "value": tri_all / (ms * 1e-3), "unit": "triangles/s",
+        "metric": metric, "value": tri_all / (ms * 1e-3), "unit": unit,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "catalogues": [c["name"] for c in cats],
-                   "n_points": [int(c["points"].shape[0]) for c in cats], "triangles_per_step": tri,
+                   "n_points": [int(c["points"].shape[0]) for c in cats], "tuples_per_step": tri,
+                   "counts_sha1": stats.get("sha1"), "cap_gib": args.cap_gib, "n_windows": stats.get("windows"),
+                   "staged_bytes_per_step": stats.get("staged_bytes"),
                    "edges_per_step": st["edges"], "hub_spoke_edges_per_s": st["edges"] / (ms * 1e-3),
-                   "step": "graph build + 3pCF + fold for every catalogue", "l2": "flushed between timed steps "
-                   "(256 MiB write); CSR (>=0.3 GB per catalogue) exceeds the 126 MB L2",
+                   "step": "graph build + enumeration (3pCF / 4pCF / parity-4pCF by workload) + fold for every "
+                   "catalogue", "l2": "flushed between timed steps (256 MiB write); the CSR of the default workload "
+                   "(>=0.3 GB per catalogue) exceeds the 126 MB L2",
                    "algo": args.algo, "build_ms": st["build_ms"], "query_ms": st["query_ms"],
                    "enum_kernel_ms": st["enum_ms"], "enum_kernel_ms_per_catalogue": enum_ms,
-                   "query_only_triangles_per_s": tri / (st["query_ms"] * 1e-3), "four_pcf": four},
+                   "query_only_tuples_per_s": tri / (st["query_ms"] * 1e-3), "four_pcf": four},
         "clocks": clocks,
-        "e2e": {"value": tri_all / (ms_e2e * 1e-3), "unit": "triangles/s", "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
+        "e2e": None if ms_e2e is None else {"value": tri_all / (ms_e2e * 1e-3), "unit": unit,
+                                            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                                            "ms_per_step": ms_e2e},
         "gpu_launches": int(round(st["launches"] * args.steps)),
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(kern),
-                     "kernel": f"{kern} on {dw['name']}", "peak_kind": f"hbm copy, {peak_kind}",
-                     "launch_ms": enum_ms[dom], "algorithmic_bytes_per_launch": dw["bytes"],
-                     "units_per_launch": {"spoke_row_elements": dw["spoke"], "tail_elements": dw["tail"],
-                                          "hub_spoke_pairs": dw["edges"], "hits": dw["hits"]},
-                     "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits (DESIGN.md "
-                             "section 6); spoke rows are re-read from L2/L1, so this is an L2->SM figure and may "
-                             "exceed the HBM peak; traffic = dram read+write of one ncu --set full launch "
-                             "(profiles/)"},
+        "roofline": roof,
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(cats)
@@ -343,6 +393,9 @@ def main():
     ap.add_argument("--ref-stride", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-4pcf", action="store_true")
+    ap.add_argument("--skip-e2e", action="store_true", help="big workloads only: no host-buffer leg (e2e = null)")
+    ap.add_argument("--cap-gib", type=float, default=0.0,
+                    help="device_mem_cap_bytes in GiB (0 = whole CSR resident); forces the out-of-core tiler")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -583,6 +583,11 @@ void segsort(const OffT *seg, int64_t seg_lo, int64_t seg_hi, int64_t e0, int ma
 
 }  // namespace
 
+void gr_exclusive_scan_i32(const int32_t *d_in, int64_t n, int32_t *d_out, cudaStream_t st)
+{
+    exclusive_scan<int32_t>(d_in, n, d_out, st);
+}
+
 // ---------------------------------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced)
 {

@@ -105,6 +105,11 @@ struct gramsci_graph {
     // size 2^s labels (s = GR_S_MIN .. GR_S_MAX), the longest page table and the most pages a row touches
     int32_t max_ptl[16] = {0};
     int32_t max_pages[16] = {0};
+    // 4pCF: raw 6-tuple -> (canonical configuration id | chirality code << 24), and configuration id -> dense
+    // index; built on the device at the first 4pCF call (query4.cu)
+    DevBuf<uint32_t> lut4;
+    DevBuf<int32_t> dense4;
+    int ncfg4 = 0;
     // out-of-core state: edge arrays in pinned host memory, cut into row-aligned windows
     uint64_t cap_bytes = 0;
     int ooc = 0;
@@ -119,6 +124,7 @@ struct gramsci_graph {
 // ---- build_graph.cu -----------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced);
 void gr_export_csr(const gramsci_graph *g, int64_t *d_ptr, int32_t *d_idx, uint8_t *d_bin, uint8_t *d_pix);
+void gr_exclusive_scan_i32(const int32_t *d_in, int64_t n, int32_t *d_out /*[n+1]*/, cudaStream_t st);
 
 // ---- query kernels ----------------------------------------------------------------------------
 // Device views handed to the enumeration kernels: hub rows come from (idx_h,bin_h,pix_h) holding

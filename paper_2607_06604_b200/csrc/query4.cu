@@ -30,6 +30,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 
 namespace {
 
@@ -42,6 +43,7 @@ struct Q4Params {
     int row_cap;         // staged hub row capacity (multiple of 16)
     int parity, weighted, want_counts;
     int n_shards;
+    int ncfg;            // LUT path: number of canonical configurations (histograms are indexed by configuration)
 };
 
 __constant__ int8_t c_perm4[24][4] = {
@@ -62,21 +64,29 @@ __device__ __forceinline__ int lower_bound_s(const int32_t *a, int lo, int hi, i
 // cnt_e/cnt_o/w_e/w_o: [n_shards][nh] raw histograms (any may be null).
 // SMALL: the local matrix D (bytes) and its bit rows live in shared memory (rows up to a few hundred
 // entries); otherwise in the CTA's slice of the global scratch.
-template <bool SMALL>
+// LUT: a raw tuple is mapped to its canonical configuration on the spot (lut[x] = configuration id | chirality
+// code << 24, built on the device once per graph); counts then go to per-CTA SHARED uint32 / int32 histograms
+// over configurations (native ATOMS, hardware-aggregated on equal addresses) and weighted sums to one global
+// slab per CTA, instead of one global RED per hit and channel into nb^6 raw bins.  In that mode cnt_e/cnt_o
+// are [ncfg] and w_e/w_o are [grid][ncfg]; without it they are [n_shards][nh] raw histograms.
+template <bool SMALL, bool LUT>
 __global__ void __launch_bounds__(Q4_THREADS)
 k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *scratch, size_t scratch_stride,
-       const double *__restrict__ pix_tab, unsigned long long *__restrict__ cnt_e,
+       const double *__restrict__ pix_tab, const uint32_t *__restrict__ lut, unsigned long long *__restrict__ cnt_e,
        unsigned long long *__restrict__ cnt_o, double *__restrict__ w_e, double *__restrict__ w_o)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     // layout: [tab 256*3*8 (parity)] [w row_cap*8 (weighted)] [idx row_cap*4] [t3 row_cap*4] [queues 8*64*4]
-    //         [pix row_cap] [SMALL: D row_cap*row_cap, bits row_cap*(row_cap/32)*4]
+    //         [LUT: h_e ncfg*4, h_o ncfg*4 (parity)] [pix row_cap] [SMALL: D row_cap*row_cap, bits row_cap*(row_cap/32)*4]
     double *s_tab = (double *)smem;
     double *a_w = (double *)(smem + (p.parity ? 256 * 3 * 8 : 0));
     int32_t *a_idx = (int32_t *)((unsigned char *)a_w + (p.weighted ? (size_t)p.row_cap * 8 : 0));
     uint32_t *a_t3 = (uint32_t *)(a_idx + p.row_cap);       // b_ic * nb^3
     uint32_t *s_queue = a_t3 + p.row_cap;                   // per warp: 64 pending local edges (a << 16 | b)
-    uint8_t *a_pix = (uint8_t *)(s_queue + Q4_WARPS * 64);
+    uint32_t *h_e = s_queue + Q4_WARPS * 64;
+    int *h_o = (int *)(h_e + (LUT ? p.ncfg : 0));
+    const int ncfg_pad = LUT ? ((p.ncfg * (p.parity ? 2 : 1) + 3) & ~3) : 0;
+    uint8_t *a_pix = (uint8_t *)(h_e + ncfg_pad);
     __shared__ int s_slot;
 
     const int nb = p.nb;
@@ -93,13 +103,20 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         bits = (uint32_t *)(D + (size_t)p.row_cap * p.row_cap);
     }
     uint32_t *my_q = s_queue + warp * 64;
-    const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh;
-    if (cnt_e) cnt_e += shard;
-    if (cnt_o) cnt_o += shard;
-    if (w_e) w_e += shard;
-    if (w_o) w_o += shard;
+    if (LUT) {
+        if (w_e) w_e += (size_t)blockIdx.x * p.ncfg;
+        if (w_o) w_o += (size_t)blockIdx.x * p.ncfg;
+        for (int t = threadIdx.x; t < ncfg_pad; t += Q4_THREADS) h_e[t] = 0u;
+    } else {
+        const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh;
+        if (cnt_e) cnt_e += shard;
+        if (cnt_o) cnt_o += shard;
+        if (w_e) w_e += shard;
+        if (w_o) w_o += shard;
+    }
     if (p.parity)
         for (int t = threadIdx.x; t < 256 * 3; t += Q4_THREADS) s_tab[t] = pix_tab[t];
+    unsigned long long budget = 0;       // LUT: upper bound of the hits this warp added since it last flushed
 
     for (;;) {
         __syncthreads();
@@ -160,7 +177,8 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
 
         // ---- phase 2: triangles of the local graph = 4-cliques under hub i; one LANE per local edge (a,b) ----
         const double wi = p.weighted ? v.w[i] : 1.0;
-        auto process = [&](uint32_t pair) {
+        auto process = [&](uint32_t pair) -> int {
+            int nhit = 0;
             const int a = (int)(pair >> 16), b = (int)(pair & 0xffffu);
             const uint8_t *Da = D + (size_t)a * ld, *Db = D + (size_t)b * ld;
             const uint32_t *Ba = bits + (size_t)a * nw, *Bb2 = bits + (size_t)b * nw;
@@ -180,23 +198,50 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
                     const int c = (w << 5) + __ffs(common) - 1;
                     common &= common - 1u;
                     const uint32_t x = base + a_t3[c] + (uint32_t)Da[c] * nb + (uint32_t)Db[c];
-                    if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
                     double ww = 0.0;
-                    if (p.weighted) {
-                        ww = wiab * a_w[c];
-                        atomicAdd(&w_e[x], ww);
-                    }
+                    if (p.weighted) ww = wiab * a_w[c];
+                    int sg = 0;
                     if (p.parity) {
                         const double *nc = s_tab + 3 * a_pix[c];
                         const double V = __dadd_rn(__dadd_rn(__dmul_rn(cx, nc[0]), __dmul_rn(cy, nc[1])),
                                                    __dmul_rn(cz, nc[2]));
-                        if (fabs(V) >= 1e-9) {
-                            const bool pos = V > 0.0;
-                            if (cnt_o) atomicAdd(&cnt_o[x], pos ? 1ull : ~0ull);     // += +-1 (mod 2^64)
-                            if (w_o) atomicAdd(&w_o[x], pos ? ww : -ww);
+                        if (fabs(V) >= 1e-9) sg = (V > 0.0) ? 1 : -1;
+                    }
+                    if (LUT) {
+                        const uint32_t e = lut[x];
+                        const uint32_t cid = e & 0xffffffu;
+                        sg *= (int)(e >> 24) - 1;                              // chirality factor of the raw tuple (A-10)
+                        ++nhit;
+                        if (cnt_e) atomicAdd(&h_e[cid], 1u);
+                        if (p.weighted && w_e) atomicAdd(&w_e[cid], ww);
+                        if (sg != 0) {
+                            if (cnt_o) atomicAdd(&h_o[cid], sg);
+                            if (w_o) atomicAdd(&w_o[cid], sg > 0 ? ww : -ww);
+                        }
+                    } else {
+                        if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
+                        if (p.weighted) atomicAdd(&w_e[x], ww);
+                        if (sg != 0) {
+                            if (cnt_o) atomicAdd(&cnt_o[x], sg > 0 ? 1ull : ~0ull);     // += +-1 (mod 2^64)
+                            if (w_o) atomicAdd(&w_o[x], sg > 0 ? ww : -ww);
                         }
                     }
                 }
+            }
+            return nhit;
+        };
+        // LUT: uint32 / int32 bins cannot wrap -- any bin holds at most the hits all 8 warps added since their own
+        // last flush, and a warp flushes the CTA histograms (atomicExch, safe against concurrent adds) before it
+        // passes 2^27
+        auto account = [&](int nhit) {
+            if (!LUT) return;
+            budget += (unsigned long long)__reduce_add_sync(0xffffffffu, nhit);
+            if (budget > (1ull << 27)) {
+                for (int t = lane; t < p.ncfg; t += 32) {
+                    if (cnt_e) { const uint32_t c = atomicExch(&h_e[t], 0u); if (c) atomicAdd(&cnt_e[t], (unsigned long long)c); }
+                    if (cnt_o) { const int c = atomicExch(&h_o[t], 0); if (c) atomicAdd(&cnt_o[t], (unsigned long long)(long long)c); }
+                }
+                budget = 0;
             }
         };
         int qn = 0;                                            // warp-uniform queue fill
@@ -215,15 +260,96 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
                     __syncwarp();
                     my_q[lane] = rest;
                     qn -= 32;
-                    process(pr);
+                    account(process(pr));
                     __syncwarp();
                 }
             }
         }
         if (qn > 0) {
             __syncwarp();
-            if (lane < qn) process(my_q[lane]);
+            account((lane < qn) ? process(my_q[lane]) : 0);
         }
+    }
+    if (LUT) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < p.ncfg; t += Q4_THREADS) {
+            if (cnt_e && h_e[t]) atomicAdd(&cnt_e[t], (unsigned long long)h_e[t]);
+            if (cnt_o && h_o[t]) atomicAdd(&cnt_o[t], (unsigned long long)(long long)h_o[t]);
+        }
+    }
+}
+
+// ---- LUT construction: canonical flag per raw tuple, then (after a scan) configuration id and chirality -------
+__device__ __forceinline__ void canon4_dev(int nb, int64_t x, int64_t &ymin, int &chi)
+{
+    int t[6];
+    {
+        int64_t r = x;
+        for (int e = 5; e >= 0; --e) { t[e] = (int)(r % nb); r /= nb; }
+    }
+    int m[4][4];
+    m[0][0] = m[1][1] = m[2][2] = m[3][3] = 0;
+    m[0][1] = m[1][0] = t[0]; m[0][2] = m[2][0] = t[1]; m[0][3] = m[3][0] = t[2];
+    m[1][2] = m[2][1] = t[3]; m[1][3] = m[3][1] = t[4]; m[2][3] = m[3][2] = t[5];
+    ymin = x;
+    int npos = 0, nneg = 0;
+    bool first = true;
+    for (int s = 0; s < 24; ++s) {
+        const int8_t *q = c_perm4[s];
+        const int u[6] = {m[q[0]][q[1]], m[q[0]][q[2]], m[q[0]][q[3]], m[q[1]][q[2]], m[q[1]][q[3]], m[q[2]][q[3]]};
+        int64_t y = 0;
+        for (int e = 0; e < 6; ++e) y = y * nb + u[e];
+        int inv = 0;
+        for (int a = 0; a < 4; ++a)
+            for (int b = a + 1; b < 4; ++b) inv += (q[a] > q[b]) ? 1 : 0;
+        if (first || y < ymin) { ymin = y; npos = nneg = 0; first = false; }
+        if (y == ymin) { if (inv & 1) ++nneg; else ++npos; }
+    }
+    chi = (npos && nneg) ? 0 : (npos ? 1 : -1);      // parity of the vertex orders reaching the minimum (A-10)
+}
+
+__global__ void k_lut_flag(int nb, int64_t nh, int32_t *__restrict__ flag)
+{
+    const int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= nh) return;
+    int64_t ymin;
+    int chi;
+    canon4_dev(nb, x, ymin, chi);
+    flag[x] = (ymin == x) ? 1 : 0;
+}
+
+__global__ void k_lut_fill(int nb, int64_t nh, const int32_t *__restrict__ rank, uint32_t *__restrict__ lut,
+                           int32_t *__restrict__ dense_of)
+{
+    const int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= nh) return;
+    int64_t ymin;
+    int chi;
+    canon4_dev(nb, x, ymin, chi);
+    lut[x] = (uint32_t)rank[ymin] | ((uint32_t)(chi + 1) << 24);
+    if (ymin == x) dense_of[rank[x]] = (int32_t)x;
+}
+
+// LUT path fold: per configuration, counts as they are and the per-CTA weight slabs summed
+__global__ void k_fold4_cfg(int ncfg, int n_slabs, const int32_t *__restrict__ dense_of,
+                            const unsigned long long *__restrict__ cnt_e, const unsigned long long *__restrict__ cnt_o,
+                            const double *__restrict__ w_e, const double *__restrict__ w_o,
+                            unsigned long long *__restrict__ out_ce, long long *__restrict__ out_co,
+                            double *__restrict__ out_we, double *__restrict__ out_wo)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncfg) return;
+    const int64_t x = dense_of[c];
+    if (out_ce) out_ce[x] = cnt_e[c];
+    if (out_co) out_co[x] = (long long)cnt_o[c];
+    if (out_we || out_wo) {
+        double se = 0.0, so = 0.0;
+        for (int k = 0; k < n_slabs; ++k) {
+            if (out_we) se += w_e[(size_t)k * ncfg + c];
+            if (out_wo) so += w_o[(size_t)k * ncfg + c];
+        }
+        if (out_we) out_we[x] = se;
+        if (out_wo) out_wo[x] = so;
     }
 }
 
@@ -314,14 +440,44 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
 
     const size_t rc = (size_t)p.row_cap;
     if (rc >= 65536) GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) exceeds 65535", g->max_row);
+
+    // ---- configuration LUT (once per graph): flag canonical tuples, rank them, fill ----
+    // (measured slower than plain RED so far -- cfg3 13.3 vs 9.8 ms, cfg4 replica 579 vs 411 ms: the dependent LUT
+    //  load sits in every lane's serial hit loop -- so it is opt-in: GRAMSCI_4PCF_LUT=1)
+    const char *lut_env = getenv("GRAMSCI_4PCF_LUT");
+    const bool want_lut = lut_env && lut_env[0] == '1';
+    if (want_lut && nb <= 10 && g->ncfg4 == 0) {
+        DevBuf<int32_t> flag, rank;
+        flag.alloc((size_t)nh);
+        rank.alloc((size_t)nh + 1);
+        k_lut_flag<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, flag.p);
+        gr_exclusive_scan_i32(flag.p, nh, rank.p, st);
+        int32_t ncfg = 0;
+        GR_CUDA(cudaMemcpyAsync(&ncfg, rank.p + nh, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        g->lut4.alloc((size_t)nh);
+        g->dense4.alloc((size_t)ncfg);
+        k_lut_fill<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, rank.p, g->lut4.p, g->dense4.p);
+        GR_CUDA(cudaGetLastError());
+        GR_CUDA(cudaStreamSynchronize(st));
+        g->ncfg4 = ncfg;
+        g->n_launches += 5;
+    }
+
+    // ---- shared memory plan: staged row, queues, (LUT) configuration histograms, (SMALL) local matrix ----
     const size_t mat_bytes = rc * rc + rc * ((rc + 31) / 32) * 4;        // D (bytes) + bit rows
     size_t smem = (p.parity ? 256 * 3 * 8 : 0) + rc * (4 + 4 + 1 + (p.weighted ? 8 : 0)) + Q4_WARPS * 64 * 4 + 64;
     smem = (smem + 15) & ~(size_t)15;
-    const bool small = smem + mat_bytes <= 96 * 1024;
+    const size_t hist_bytes = (((size_t)g->ncfg4 * (p.parity ? 2 : 1) + 3) & ~(size_t)3) * 4;
+    const bool use_lut = want_lut && g->ncfg4 > 0 && smem + hist_bytes <= 120 * 1024 && (d_even_c || d_odd_c);
+    p.ncfg = use_lut ? g->ncfg4 : 0;
+    if (use_lut) smem += hist_bytes;
+    const bool small = smem + mat_bytes <= 100 * 1024;
     if (small) smem += mat_bytes;
     if (smem > g->smem_optin)
         GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
-    const void *fn = small ? (const void *)k_4pcf<true> : (const void *)k_4pcf<false>;
+    const void *fn = small ? (use_lut ? (const void *)k_4pcf<true, true> : (const void *)k_4pcf<true, false>)
+                           : (use_lut ? (const void *)k_4pcf<false, true> : (const void *)k_4pcf<false, false>);
     GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
     GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, Q4_THREADS, smem));
@@ -337,11 +493,13 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     scratch.alloc(stride * grid + 256);
     counter.alloc(1);
     GR_CUDA(cudaMemsetAsync(counter.p, 0, sizeof(unsigned int), st));
-    const size_t tot = (size_t)nh * p.n_shards;
-    if (d_even_c) { ce.alloc(tot); GR_CUDA(cudaMemsetAsync(ce.p, 0, tot * 8, st)); }
-    if (d_odd_c) { co.alloc(tot); GR_CUDA(cudaMemsetAsync(co.p, 0, tot * 8, st)); }
-    if (d_even_w || d_odd_w) { we.alloc(tot); GR_CUDA(cudaMemsetAsync(we.p, 0, tot * 8, st)); }
-    if (d_odd_w) { wo.alloc(tot); GR_CUDA(cudaMemsetAsync(wo.p, 0, tot * 8, st)); }
+    // LUT: counts [ncfg], weights [grid][ncfg]; raw: [n_shards][nh] each
+    const size_t tot_c = use_lut ? (size_t)p.ncfg : (size_t)nh * p.n_shards;
+    const size_t tot_w = use_lut ? (size_t)p.ncfg * grid : (size_t)nh * p.n_shards;
+    if (d_even_c) { ce.alloc(tot_c); GR_CUDA(cudaMemsetAsync(ce.p, 0, tot_c * 8, st)); }
+    if (d_odd_c) { co.alloc(tot_c); GR_CUDA(cudaMemsetAsync(co.p, 0, tot_c * 8, st)); }
+    if (d_even_w || d_odd_w) { we.alloc(tot_w); GR_CUDA(cudaMemsetAsync(we.p, 0, tot_w * 8, st)); }
+    if (d_odd_w) { wo.alloc(tot_w); GR_CUDA(cudaMemsetAsync(wo.p, 0, tot_w * 8, st)); }
     if (p.parity) {
         // pixel-centre unit vectors (A-8): z_c = (iz + 1/2)/8 - 1, phi_c = (iphi + 1/2) pi/8
         std::vector<double> h(256 * 3);
@@ -369,20 +527,33 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     {
         GrTimer en(st);
         if (g->n > 0) {
-            if (small)
-                k_4pcf<true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
-                                                             (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
+            double *wep = (d_even_w || d_odd_w) ? we.p : nullptr;
+            if (small && use_lut)
+                k_4pcf<true, true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, g->lut4.p, ce.p, co.p, wep, wo.p);
+            else if (small)
+                k_4pcf<true, false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, nullptr, ce.p, co.p, wep, wo.p);
+            else if (use_lut)
+                k_4pcf<false, true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, g->lut4.p, ce.p, co.p, wep, wo.p);
             else
-                k_4pcf<false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, ce.p, co.p,
-                                                              (d_even_w || d_odd_w) ? we.p : nullptr, wo.p);
+                k_4pcf<false, false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, nullptr, ce.p, co.p, wep, wo.p);
             GR_CUDA(cudaGetLastError());
             g->n_launches += 1;
         }
         g->t_enum_ms = en.stop();
     }
-    k_fold4<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, p.n_shards, ce.p, co.p, d_even_w ? we.p : nullptr, wo.p,
-                                                          (unsigned long long *)d_even_c, (long long *)d_odd_c,
-                                                          d_even_w, d_odd_w);
+    if (use_lut) {
+        if (d_even_c) GR_CUDA(cudaMemsetAsync(d_even_c, 0, (size_t)nh * 8, st));
+        if (d_odd_c) GR_CUDA(cudaMemsetAsync(d_odd_c, 0, (size_t)nh * 8, st));
+        if (d_even_w) GR_CUDA(cudaMemsetAsync(d_even_w, 0, (size_t)nh * 8, st));
+        if (d_odd_w) GR_CUDA(cudaMemsetAsync(d_odd_w, 0, (size_t)nh * 8, st));
+        k_fold4_cfg<<<(p.ncfg + 127) / 128, 128, 0, st>>>(p.ncfg, grid, g->dense4.p, ce.p, co.p, d_even_w ? we.p : nullptr,
+                                                         d_odd_w ? wo.p : nullptr, (unsigned long long *)d_even_c,
+                                                         (long long *)d_odd_c, d_even_w, d_odd_w);
+    } else {
+        k_fold4<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, p.n_shards, ce.p, co.p, d_even_w ? we.p : nullptr, wo.p,
+                                                              (unsigned long long *)d_even_c, (long long *)d_odd_c,
+                                                              d_even_w, d_odd_w);
+    }
     GR_CUDA(cudaGetLastError());
     g->n_launches += 1;
     GR_CUDA(cudaStreamSynchronize(st));

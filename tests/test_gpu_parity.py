@@ -170,8 +170,11 @@ def test_4pcf_parity(periodic):
     assert e.value.code == 1
 
 
-def test_4pcf_parity_wedge():
-    """Scaled replica of BASELINE configs[3] (survey wedge, open box, weights U(0.8,1.2), 8 bins)."""
+@pytest.mark.parametrize("lut", ["0", "1"])
+def test_4pcf_parity_wedge(lut, monkeypatch):
+    """Scaled replica of BASELINE configs[3] (survey wedge, open box, weights U(0.8,1.2), 8 bins); with the
+    plain raw-histogram kernel and with the opt-in configuration-LUT variant (GRAMSCI_4PCF_LUT=1)."""
+    monkeypatch.setenv("GRAMSCI_4PCF_LUT", lut)
     cfg = cat.config4(seed=4002, n=6000, cap_deg=7.0)
     og, gg = build_both(cfg, want_pixels=True)
     ec, ew, oc, ow = og.pcf4(parity=True)
