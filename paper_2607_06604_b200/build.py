@@ -17,7 +17,7 @@ HEADERS = [os.path.join(CSRC, "internal.cuh"), os.path.join(HERE, "..", "include
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--fmad=false",                      # A-3/A-9: no FMA contraction anywhere in the device code
-    "-Xcompiler", "-fPIC,-O2,-ffp-contract=off",
+    "-Xcompiler", "-fPIC,-O2,-ffp-contract=off,-pthread",
     "-Xptxas", "-v",
 ]
 
@@ -54,7 +54,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.returncode != 0:
             sys.stderr.write(out)
             raise RuntimeError(f"nvcc failed on {s}")
-    cmd = [_nvcc(), "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB, *objs, "-lcudart"]
+    cmd = [_nvcc(), "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB, *objs, "-lcudart", "-lpthread"]
     subprocess.run(cmd, check=True)
     with open(os.path.join(CSRC, "ptxas_info.log"), "w") as f:
         f.write("\n".join(log))

@@ -8,6 +8,10 @@
 #include <cstring>
 #include <map>
 #include <mutex>
+#include <thread>
+#include <vector>
+#include <algorithm>
+#include <sys/mman.h>
 
 // ---- errors --------------------------------------------------------------------------------------------
 static thread_local char t_err[512] = "";
@@ -54,6 +58,41 @@ bool gr_pools_supported()
         if (state < 0) { state = 0; cudaGetLastError(); }
     }
     return state == 1;
+}
+
+// ---- page-locked host memory -------------------------------------------------------------------------------
+void *gr_pinned_alloc(size_t bytes)
+{
+    bytes = (bytes + 4095) & ~size_t(4095);
+    void *p = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+    if (p == MAP_FAILED) GR_FAIL(GRAMSCI_ENOMEM, "out-of-core: cannot map %zu bytes of host memory", bytes);
+    madvise(p, bytes, MADV_HUGEPAGE);
+    unsigned nt = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
+    if (bytes < (size_t(64) << 20)) nt = 1;
+    std::vector<std::thread> th;
+    const size_t chunk = ((bytes / nt) + 4095) & ~size_t(4095);
+    for (unsigned t = 0; t < nt; ++t)
+        th.emplace_back([=] {
+            char *c = (char *)p;
+            const size_t lo = std::min(bytes, (size_t)t * chunk), hi = std::min(bytes, lo + chunk);
+            for (size_t o = lo; o < hi; o += 4096) c[o] = 0;
+        });
+    for (auto &t : th) t.join();
+    cudaError_t e = cudaHostRegister(p, bytes, cudaHostRegisterDefault);
+    if (e != cudaSuccess) {
+        munmap(p, bytes);
+        cudaGetLastError();
+        GR_FAIL(GRAMSCI_ENOMEM, "out-of-core: cannot page-lock %zu bytes of host memory (%s)", bytes, cudaGetErrorString(e));
+    }
+    return p;
+}
+
+void gr_pinned_free(void *p, size_t bytes)
+{
+    if (!p) return;
+    bytes = (bytes + 4095) & ~size_t(4095);
+    cudaHostUnregister(p);
+    munmap(p, bytes);
 }
 
 // ---- pointer staging -------------------------------------------------------------------------------------
@@ -167,10 +206,20 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->cap_bytes = o.device_mem_cap_bytes;
     int dev = 0;
     GR_CUDA(cudaGetDevice(&dev));
-    cudaDeviceProp prop;
-    GR_CUDA(cudaGetDeviceProperties(&prop, dev));
-    g->sm_count = prop.multiProcessorCount;
-    g->smem_optin = prop.sharedMemPerBlockOptin;
+    {   // two attributes, cached per device (cudaGetDeviceProperties costs milliseconds per call)
+        static std::mutex mu;
+        static std::map<int, std::pair<int, size_t>> cache;
+        std::lock_guard<std::mutex> lk(mu);
+        auto it = cache.find(dev);
+        if (it == cache.end()) {
+            int sms = 0, optin = 0;
+            GR_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            GR_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+            it = cache.emplace(dev, std::make_pair(sms, (size_t)optin)).first;
+        }
+        g->sm_count = it->second.first;
+        g->smem_optin = it->second.second;
+    }
 
     gr_alloc_stream() = g->stream;
     DevBuf<double> hp, hw;
@@ -191,9 +240,9 @@ extern "C" void gramsci_free_graph(gramsci_graph *g)
 {
     if (!g) return;
     cudaStreamSynchronize(g->stream);
-    if (g->h_idx) cudaFreeHost(g->h_idx);
-    if (g->h_bin) cudaFreeHost(g->h_bin);
-    if (g->h_pix) cudaFreeHost(g->h_pix);
+    gr_pinned_free(g->h_idx, g->h_idx_bytes);
+    gr_pinned_free(g->h_bin, g->h_bin_bytes);
+    gr_pinned_free(g->h_pix, g->h_pix_bytes);
     delete g;
 }
 

@@ -769,10 +769,14 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         launches += 1;
         GR_CUDA(cudaGetLastError());
     } else {
-        GR_CUDA(cudaHostAlloc((void **)&g->h_idx, std::max<size_t>((size_t)E * 4 + 256, 256), cudaHostAllocDefault));
-        GR_CUDA(cudaHostAlloc((void **)&g->h_bin, std::max<size_t>((size_t)E + 256, 256), cudaHostAllocDefault));
-        if (g->has_pix)
-            GR_CUDA(cudaHostAlloc((void **)&g->h_pix, std::max<size_t>((size_t)E + 256, 256), cudaHostAllocDefault));
+        g->h_idx_bytes = std::max<size_t>((size_t)E * 4 + 256, 256);
+        g->h_bin_bytes = std::max<size_t>((size_t)E + 256, 256);
+        g->h_idx = (int32_t *)gr_pinned_alloc(g->h_idx_bytes);
+        g->h_bin = (uint8_t *)gr_pinned_alloc(g->h_bin_bytes);
+        if (g->has_pix) {
+            g->h_pix_bytes = g->h_bin_bytes;
+            g->h_pix = (uint8_t *)gr_pinned_alloc(g->h_pix_bytes);
+        }
         int64_t maxlen = 0;
         for (auto &w : g->windows) maxlen = std::max(maxlen, w.e_hi - w.e_lo);
         DevBuf<int32_t> widx;

@@ -117,9 +117,15 @@ struct gramsci_graph {
     std::vector<uint8_t> need;     // [W*W] need[h*W+c] = 1 iff some edge (i,j) has i in window h, j in window c
     int32_t *h_idx = nullptr;      // pinned [E]
     uint8_t *h_bin = nullptr, *h_pix = nullptr;
+    size_t h_idx_bytes = 0, h_bin_bytes = 0, h_pix_bytes = 0;
     // timing of the last calls
     double t_build_ms = 0, t_query_ms = 0, t_enum_ms = 0, n_launches = 0, staged_bytes = 0;
 };
+
+// page-locked host memory for the out-of-core windows (api.cu): anonymous mapping, pages touched by all
+// host cores, then cudaHostRegister -- cudaHostAlloc pins at 2.6 GiB/s on this box, this path at ~25 GiB/s
+void *gr_pinned_alloc(size_t bytes);
+void gr_pinned_free(void *p, size_t bytes);
 
 // ---- build_graph.cu -----------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced);
