@@ -1,6 +1,8 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Integer counts bit-exact; fp64 weighted sums within 1e-10 relative
 (BASELINE.json north_star; per-bin scale = sum of |prod w|, S:8(c) A-13)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -284,3 +286,78 @@ def test_out_of_core_cap_derives_windows():
     assert np.array_equal(g1.pcf3()[0], og.pcf3()[0])
     with pytest.raises(gr.GramsciError):
         g1.pcf4()
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times ------------------------------------
+@pytest.mark.slow
+@pytest.mark.parametrize("which", ["cfg2R", "cfg2D"])
+def test_full_size_config2_matches_oracle(which):
+    """configs[1] in full (1e6 points per catalogue, device-resident inputs, default algo = what bench.py
+    times): every bin of the 3pCF against the full oracle run (about 10 s of host time on 16 cores)."""
+    cfg = cat.config2_randoms() if which == "cfg2R" else cat.config2_data()
+    og, gg = build_both(cfg)
+    assert gg.info()["n_edges"] == og.n_edges
+    oc, ow = og.pcf3()
+    weighted = cfg["weights"] is not None
+    c, w = gg.pcf3(weighted=weighted)
+    assert c.sum() == oc.sum() and np.array_equal(c, oc)
+    if weighted:
+        assert_weighted_close(w, ow)
+    assert np.array_equal(gg.pcf2()[0], og.pcf2()[0])
+
+
+@pytest.mark.slow
+def test_full_size_config3_matches_oracle():
+    """configs[2] in full (2e5 points, 1.5e9 tetrahedra): every bin of the 4pCF, the 3pCF and the 2pCF of the
+    same graph against the full oracle run; relabelling invariance (C-3) on the GPU path at full size; the
+    total on the Monte-Carlo 4-clique density of a Poisson field (C-6)."""
+    cfg = cat.config3()
+    og = oracle.Graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    oc, _ = og.pcf4()
+    gg = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    c, _ = gg.pcf4()
+    assert c.sum() == oc.sum() > 1e9
+    assert np.array_equal(c, oc)
+    assert np.array_equal(gg.pcf3()[0], og.pcf3()[0])
+    assert np.array_equal(gg.pcf2()[0], og.pcf2()[0])
+    perm = np.random.default_rng(7).permutation(og.n)
+    g2 = gr.gramsci_build_graph(np.ascontiguousarray(cfg["points"][perm]), None, cfg["box"], cfg["r_min"],
+                                cfg["r_max"], cfg["nbins"])
+    assert np.array_equal(g2.pcf4()[0], c)
+    # Poisson 4-clique density: N m^3 p4 / 24 with p4 = 0.1582 +- 0.0002 (Monte Carlo, SURVEY 8(c) C-6)
+    m = 2.0 * og.n_edges / og.n
+    assert abs(c.sum() / (og.n * m ** 3 * 0.1582 / 24.0) - 1.0) < 0.01
+
+
+@pytest.mark.slow
+def test_full_size_config4_replica_parity_matches_oracle():
+    """1/8 replica of configs[3] (62,500 points in a 15 x 15 degree wedge, same density and radii, weights
+    U(0.8,1.2), 2.1e10 tetrahedra): all four channels of the parity-decomposed 4pCF against the full oracle."""
+    cfg = cat.config4(n=62_500, cap_deg=15.0)
+    og = oracle.Graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    gg = gr.gramsci_build_graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                want_pixels=True)
+    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
+    assert gec.sum() == ec.sum() > 1e10
+    assert np.array_equal(gec, ec) and np.array_equal(goc, oc)
+    assert_weighted_close(gew, ew)
+    assert_weighted_close(gow, ow, scale=np.abs(ew))
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("GRAMSCI_TEST_FULL_CFG4") != "1",
+                    reason="about 10 minutes of host time for the oracle; set GRAMSCI_TEST_FULL_CFG4=1")
+def test_full_size_config4_parity_matches_oracle():
+    """configs[3] in full (5e5 points, 1.7e11 tetrahedra, weighted, even and odd channels)."""
+    cfg = cat.config4()
+    og = oracle.Graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    gg = gr.gramsci_build_graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                want_pixels=True)
+    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
+    print("cfg4 full: tetrahedra", int(gec.sum()), "query ms", gg.timing(1), "sum|odd|", int(np.abs(goc).sum()))
+    assert gec.sum() == ec.sum() > 1e11
+    assert np.array_equal(gec, ec) and np.array_equal(goc, oc)
+    assert_weighted_close(gew, ew)
+    assert_weighted_close(gow, ow, scale=np.abs(ew))
