@@ -77,6 +77,10 @@ typedef struct {       /* zero-initialised struct == defaults */
     int algo;                      /* GRAMSCI_ALGO_* for gramsci_3pcf                                      */
     int n_windows;                 /* out-of-core only: force this many row windows (0 = derive from cap);
                                       the paper's env-var override, P:159                                 */
+    int hub_stride;                /* > 1: enumerate only tuples whose smallest-label vertex i has i % hub_stride
+                                      == 0 (a sampled partial result, for checking full-size runs against a
+                                      reference that is too slow to run in full); needs caller labels
+                                      (relabel = 2 or want_pixels), else GRAMSCI_EINVAL                    */
 } gramsci_options;
 
 /*

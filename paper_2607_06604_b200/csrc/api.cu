@@ -171,7 +171,7 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     gramsci_options o;
     memset(&o, 0, sizeof o);
     if (opt) o = *opt;
-    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0)
+    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0 || o.hub_stride < 0)
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: bad options");
     require_device();
 
@@ -202,6 +202,11 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->has_pix = o.want_pixels ? 1 : 0;
     g->spatial = (o.relabel == 1) ? 1 : (o.relabel == 2) ? 0 : (o.want_pixels ? 0 : 1);
     g->algo = o.algo;
+    g->hub_stride = o.hub_stride > 1 ? o.hub_stride : 1;
+    if (g->hub_stride > 1 && g->spatial) {
+        delete g; g = nullptr;
+        GR_FAIL(GRAMSCI_EINVAL, "build_graph: hub_stride needs caller labels (relabel = 2 or want_pixels)");
+    }
     g->stream = (cudaStream_t)o.stream;
     g->cap_bytes = o.device_mem_cap_bytes;
     int dev = 0;

@@ -85,7 +85,7 @@ struct gramsci_graph {
     double box[3] = {0, 0, 0};
     double r_min = 0, r_max = 0;
     double q[GR_MAXBINS + 1];      // squared bin edges (A-3)
-    int weighted = 0, has_pix = 0, spatial = 0, algo = 0;
+    int weighted = 0, has_pix = 0, spatial = 0, algo = 0, hub_stride = 1;
     cudaStream_t stream = nullptr;
     int sm_count = GR_SM_COUNT_FALLBACK;
     size_t smem_optin = 0;
@@ -145,6 +145,7 @@ struct GrView {
     const int32_t *order;   // hub schedule (labels in spatial order), [n]
     int32_t s_lo, s_hi;     // schedule slots to walk (in-core: [0,n))
     const double *w;        // weights by label or nullptr
+    int32_t hub_stride;     // > 1: only hubs with label % hub_stride == 0
 };
 
 void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);

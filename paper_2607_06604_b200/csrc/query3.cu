@@ -78,7 +78,7 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
         const int s = s_slot;
         if (s >= v.s_hi) break;
         const int32_t i = v.order[s];
-        const bool mine = (i >= v.h_lo && i < v.h_hi);
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n >= 2) {
@@ -249,7 +249,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             if (s_cur >= v.s_hi) break;
         }
         const int32_t i = v.order[s_cur++];
-        const bool mine = (i >= v.h_lo && i < v.h_hi);
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n < 2) continue;
@@ -633,7 +633,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         if (best_s >= 0) {
             const size_t soft = 100 * 1024;       // two CTAs per SM
             int G = 0;
-            const int forced = (g->algo >= GRAMSCI_ALGO_TABLE_G1) ? (1 << (g->algo - GRAMSCI_ALGO_TABLE_G1)) : 0;
+            const int forced = (g->algo >= GRAMSCI_ALGO_TABLE_G1 && g->algo <= GRAMSCI_ALGO_TABLE_G8) ? (1 << (g->algo - GRAMSCI_ALGO_TABLE_G1)) : 0;
             for (int cand = 1; cand <= 8 && !G; cand *= 2) {
                 if (forced && cand != forced) continue;
                 const size_t cta = hist_bytes + (size_t)(Q3_WARPS / cand) * table_group_bytes(g, best_s, W, cand, r.p.row_cap, &ptl, &tbl);
@@ -681,7 +681,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     counter.alloc(1);
     raw_cnt.alloc((size_t)nh);
     GR_CUDA(cudaMemsetAsync(raw_cnt.p, 0, sizeof(unsigned long long) * nh, st));
-    const int n_slots = r.grid;                         // one fp64 slab per CTA
+    const int n_slots = r.grid;                         // one fp64 slab per CTA (weighted only)
     if (W) {
         raw_w.alloc((size_t)nh * n_slots);
         GR_CUDA(cudaMemsetAsync(raw_w.p, 0, sizeof(double) * (size_t)nh * n_slots, st));

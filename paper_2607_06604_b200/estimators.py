@@ -1,0 +1,38 @@
+"""Host-side post-processing above the hot path (S:8(f) rank 1; sec. 3.3): NumPy arithmetic on
+the histograms the CUDA library returns.  Nothing here enumerates tuples.
+
+* :func:`xi_periodic`      -- 2pCF of a periodic box without randoms (reading A-12, mode b)
+* :func:`zeta3_ratio`      -- zeta = NNN / RRR per configuration from a (weighted) data and a random 3pCF
+* :func:`zeta4_connected`  -- Eq. 5: zeta_conn = zeta - zeta_disc, zeta_disc from Eq. 4 (``gramsci_zeta_disc``)
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def bin_edges(r_min: float, r_max: float, nbins: int) -> np.ndarray:
+    return r_min + np.arange(nbins + 1) * (r_max - r_min) / nbins
+
+
+def xi_periodic(cnt2: np.ndarray, n: int, box, r_min: float, r_max: float) -> np.ndarray:
+    """xi_b = cnt2_b / [C(N,2) (4 pi/3)(e_{b+1}^3 - e_b^3)/V] - 1 for a periodic box (A-12 b)."""
+    e = bin_edges(r_min, r_max, cnt2.size)
+    rr = 0.5 * n * (n - 1) * (4.0 * np.pi / 3.0) * (e[1:] ** 3 - e[:-1] ** 3) / float(np.prod(box))
+    return np.asarray(cnt2, dtype=np.float64) / rr - 1.0
+
+
+def zeta3_ratio(data_hist: np.ndarray, data_norm: float, rand_hist: np.ndarray, rand_norm: float) -> np.ndarray:
+    """NNN/RRR per bin: (data_hist / data_norm^3) / (rand_hist / rand_norm^3); data_norm = sum of the data
+    weights (or N for unit weights), rand_norm likewise.  Bins with an empty random histogram give NaN."""
+    num = np.asarray(data_hist, dtype=np.float64) / float(data_norm) ** 3
+    den = np.asarray(rand_hist, dtype=np.float64) / float(rand_norm) ** 3
+    out = np.full(num.shape, np.nan)
+    np.divide(num, den, out=out, where=den != 0)
+    return out
+
+
+def zeta4_connected(zeta4: np.ndarray, xi: np.ndarray) -> np.ndarray:
+    """Eq. 5: zeta_conn = zeta - zeta_disc on the dense [nb^6] layout, zeta_disc from Eq. 4 through
+    the library's host helper.  Applies to the even channel only."""
+    from . import gramsci_zeta_disc
+    return np.asarray(zeta4, dtype=np.float64) - gramsci_zeta_disc(np.asarray(xi, dtype=np.float64))

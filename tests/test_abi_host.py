@@ -90,3 +90,19 @@ def test_product_never_imports_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in src.replace("the oracle", "").replace("oracle's", ""), f
+
+
+def test_estimator_helpers(lib):
+    from paper_2607_06604_b200 import estimators as est
+    # a periodic Poisson box has xi = 0 when the pair counts sit on their expectation
+    n, box, nb = 1000, [50.0, 50.0, 50.0], 4
+    e = est.bin_edges(0.0, 8.0, nb)
+    expect = 0.5 * n * (n - 1) * (4 * np.pi / 3) * (e[1:] ** 3 - e[:-1] ** 3) / 50.0 ** 3
+    assert np.allclose(est.xi_periodic(expect, n, box, 0.0, 8.0), 0.0)
+    # NNN/RRR: doubling every data weight multiplies the histogram by 8 and the norm by 2 -> same zeta
+    h = np.arange(1, 9, dtype=np.float64)
+    assert np.allclose(est.zeta3_ratio(8 * h, 2 * 10.0, h, 10.0), 1.0)
+    assert np.isnan(est.zeta3_ratio(h, 1.0, np.zeros(8), 1.0)).all()
+    # Eq. 5 with xi = 0 leaves zeta untouched
+    z = np.random.default_rng(1).normal(size=3 ** 6)
+    assert np.array_equal(est.zeta4_connected(z, np.zeros(3)), z)

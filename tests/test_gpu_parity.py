@@ -245,7 +245,7 @@ def _bao_replica():
     return _BAO["cfg"], _BAO["cnt"]
 
 
-@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH])
+@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G8])
 def test_3pcf_bao_replica(algo):
     """Shrunk replica of BASELINE configs[4] (same radii and bins, L=310, 40 % of the density so that
     the oracle finishes in seconds): rows of thousands of entries, r_min > 0, 18 bins, a periodic grid
@@ -331,8 +331,9 @@ def test_full_size_config3_matches_oracle():
 
 @pytest.mark.slow
 def test_full_size_config4_replica_parity_matches_oracle():
-    """1/8 replica of configs[3] (62,500 points in a 15 x 15 degree wedge, same density and radii, weights
-    U(0.8,1.2), 2.1e10 tetrahedra): all four channels of the parity-decomposed 4pCF against the full oracle."""
+    """Reduced configs[3] (62,500 points in a 15 x 15 degree wedge -- an eighth of the points in a quarter of the
+    solid angle, i.e. half the density -- same radii, bins and weights U(0.8,1.2); 2.1e10 tetrahedra): all four
+    channels of the parity-decomposed 4pCF against the full oracle."""
     cfg = cat.config4(n=62_500, cap_deg=15.0)
     og = oracle.Graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"])
     ec, ew, oc, ow = og.pcf4(parity=True)
@@ -346,18 +347,62 @@ def test_full_size_config4_replica_parity_matches_oracle():
 
 
 @pytest.mark.slow
-@pytest.mark.skipif(os.environ.get("GRAMSCI_TEST_FULL_CFG4") != "1",
-                    reason="about 10 minutes of host time for the oracle; set GRAMSCI_TEST_FULL_CFG4=1")
-def test_full_size_config4_parity_matches_oracle():
-    """configs[3] in full (5e5 points, 1.7e11 tetrahedra, weighted, even and odd channels)."""
+def test_full_size_config4_parity_sampled_hubs():
+    """configs[3] in full (5e5 points, 1.54e12 tetrahedra, weighted, even and odd channels).  The full oracle run
+    would take more than an hour of host time, so the oracle enumerates the tetrahedra whose smallest-label vertex
+    is a multiple of 128 and the CUDA path is asked for exactly that partial result (``hub_stride``), on the graph
+    and in the launch configuration of the full run; the full run itself must contain the partial one."""
     cfg = cat.config4()
+    stride = 128
     og = oracle.Graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"])
-    ec, ew, oc, ow = og.pcf4(parity=True)
-    gg = gr.gramsci_build_graph(cfg["points"], cfg["weights"], None, cfg["r_min"], cfg["r_max"], cfg["nbins"],
-                                want_pixels=True)
-    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
-    print("cfg4 full: tetrahedra", int(gec.sum()), "query ms", gg.timing(1), "sum|odd|", int(np.abs(goc).sum()))
-    assert gec.sum() == ec.sum() > 1e11
+    ec, ew, oc, ow = og.pcf4(parity=True, hubs=(0, og.n, stride))
+    pts = _torch().from_numpy(cfg["points"]).cuda()
+    w = _torch().from_numpy(cfg["weights"]).cuda()
+    gs = gr.gramsci_build_graph(pts, w, None, cfg["r_min"], cfg["r_max"], cfg["nbins"], want_pixels=True, hub_stride=stride)
+    assert gs.info()["n_edges"] == og.n_edges
+    gec, goc, gew, gow = gs.pcf4_parity(weighted=True)
+    assert gec.sum() == ec.sum() > 5e9
     assert np.array_equal(gec, ec) and np.array_equal(goc, oc)
     assert_weighted_close(gew, ew)
     assert_weighted_close(gow, ow, scale=np.abs(ew))
+    # the same graph without the hub filter = what bench.py --workload cfg4 times
+    gf = gr.gramsci_build_graph(pts, w, None, cfg["r_min"], cfg["r_max"], cfg["nbins"], want_pixels=True)
+    fec, foc, few, fow = gf.pcf4_parity(weighted=True)
+    assert fec.sum() > 1e12 and np.all(fec >= gec) and np.all(few >= gew * (1 - 1e-12))
+    big = fec > 50_000_000
+    assert big.sum() > 100 and np.allclose(gec[big] / fec[big], 1.0 / stride, rtol=0.1)
+    # 3pCF and 2pCF of the same (caller-label) graph against the oracle, hub-sampled and in full
+    assert np.array_equal(gs.pcf3()[0], og.pcf3(hubs=(0, og.n, stride))[0])
+    assert np.array_equal(gf.pcf2()[0], og.pcf2()[0])
+
+
+def test_hub_stride_partial_results():
+    cfg = small(41, n=3000, L=30.0, weighted=True, r_max=5.0, nb=4)
+    og = oracle.Graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    for algo in (gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4):
+        g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                   relabel=2, hub_stride=7, algo=algo)
+        assert np.array_equal(g.pcf3()[0], og.pcf3(hubs=(0, og.n, 7))[0])
+        assert np.array_equal(g.pcf4()[0], og.pcf4(hubs=(0, og.n, 7))[0])
+    with pytest.raises(gr.GramsciError) as e:
+        gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], hub_stride=7)
+    assert e.value.code == 1
+
+
+def test_ddd_over_rrr_poisson_is_one():
+    """BASELINE north_star: for Poisson points in a periodic box DDD/RRR -> 1 within shot noise.  Two independent
+    uniform catalogues through the CUDA path and the host estimator helper (NNN/RRR per configuration)."""
+    from paper_2607_06604_b200 import estimators as est
+    n, L, nb = 60_000, 300.0, 6
+    d = cat.uniform_box(n, L, 61)
+    r = cat.uniform_box(2 * n, L, 62)
+    gd = gr.gramsci_build_graph(d, None, [L, L, L], 0.0, 20.0, nb)
+    grr = gr.gramsci_build_graph(r, None, [L, L, L], 0.0, 20.0, nb)
+    cd, _ = gd.pcf3()
+    cr, _ = grr.pcf3()
+    zeta = est.zeta3_ratio(cd, n, cr, 2 * n)
+    ok = cd > 20_000
+    assert ok.sum() >= 20
+    # relative scatter of a triangle count ~ a few / sqrt(count) (triples share pairs)
+    assert np.all(np.abs(zeta[ok] - 1.0) < 12.0 / np.sqrt(cd[ok]) + 12.0 / np.sqrt(cr[ok]))
+    assert abs(np.nansum(cd) / n ** 3 / (np.nansum(cr) / (2 * n) ** 3) - 1.0) < 5e-3
