@@ -33,9 +33,9 @@ import catalogues as cat  # noqa: E402
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on cfg2, from the committed
-# ncu --set full capture (profiles/r1_b_table_3pcf_full.md)
-DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 578.146816e6 + 6.029568e6,
-                      "k_3pcf_table<counts>": 301.713408e6 + 4.563456e6}
+# ncu --set full capture (profiles/r1_c_table_3pcf_full.md)
+DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 577.233152e6 + 5.401344e6,
+                      "k_3pcf_table<counts>": 302.012672e6 + 4.176896e6}
 
 
 RED_PEAK_GOPS = 186.0      # global RED.E.ADD.(U64|F64), spread addresses, all SMs (measured, see above)
