@@ -406,3 +406,50 @@ def test_ddd_over_rrr_poisson_is_one():
     # relative scatter of a triangle count ~ a few / sqrt(count) (triples share pairs)
     assert np.all(np.abs(zeta[ok] - 1.0) < 12.0 / np.sqrt(cd[ok]) + 12.0 / np.sqrt(cr[ok]))
     assert abs(np.nansum(cd) / n ** 3 / (np.nansum(cr) / (2 * n) ** 3) - 1.0) < 5e-3
+
+
+@pytest.mark.slow
+def test_full_size_config5_invariants_and_cap():
+    """configs[4] in full (2.5e6 points, 8.4e9 edges, 42 GB of CSR, 7.1e12 triangles; about two minutes on a
+    B200).  No oracle run is feasible at this size, so the result is checked through properties that hold at
+    any size: pair and triangle counts per configuration on their Poisson expectations (C-6; a periodic
+    uniform box), and the run under a 24 GiB device-memory cap bit-identical to the resident run (C-13)."""
+    torch = _torch()
+    free, _ = torch.cuda.mem_get_info()
+    try:
+        host_gb = os.sysconf("SC_PHYS_PAGES") * os.sysconf("SC_PAGE_SIZE") / 2 ** 30
+    except (ValueError, OSError):
+        host_gb = 0.0
+    if free < 70 * 2 ** 30 or host_gb < 80:
+        pytest.skip("needs 70 GiB of free device memory and 80 GiB of host memory")
+    cfg = cat.config5()
+    n, L, nb = cfg["points"].shape[0], float(cfg["box"][0]), cfg["nbins"]
+    pts = torch.from_numpy(cfg["points"]).cuda()
+    g = gr.gramsci_build_graph(pts, None, cfg["box"], cfg["r_min"], cfg["r_max"], nb)
+    e = cfg["r_min"] + np.arange(nb + 1) * (cfg["r_max"] - cfg["r_min"]) / nb
+    V = L ** 3
+    c2, _ = g.pcf2()
+    exp2 = 0.5 * n * (n - 1) * (4 * np.pi / 3) * (e[1:] ** 3 - e[:-1] ** 3) / V
+    assert c2.sum() == g.info()["n_edges"] > 8.3e9
+    assert np.all(np.abs(c2 / exp2 - 1.0) < 5e-4)
+    c3, _ = g.pcf3()
+    g.free()
+    c3r = c3.reshape(nb, nb, nb)
+    I = (e[1:] ** 2 - e[:-1] ** 2) / 2
+    worst, checked = 0.0, 0
+    for a in range(nb):
+        for b in range(a, nb):
+            for c in range(b, nb):
+                assert c3r[b, a, c] == 0 or a == b                     # populated at sorted triples only (A-5)
+                if e[c + 1] <= e[a] + e[b]:                             # triangle inequality holds on the whole bins
+                    mu = 6 if a < b < c else (1 if a == c else 3)
+                    exp3 = n * (n - 1) * (n - 2) / 6 / V ** 2 * mu * 8 * np.pi ** 2 * I[a] * I[b] * I[c]
+                    worst = max(worst, abs(c3r[a, b, c] / exp3 - 1.0))
+                    checked += 1
+    assert checked > 1000 and worst < 2e-3, (checked, worst)
+    assert 7.0e12 < c3.sum() < 7.2e12
+    g2 = gr.gramsci_build_graph(pts, None, cfg["box"], cfg["r_min"], cfg["r_max"], nb, device_mem_cap_bytes=24 * 2 ** 30)
+    assert g2.info()["n_windows"] >= 4
+    c3c, _ = g2.pcf3()
+    assert g2.timing(4) > 40e9                                          # the windows really were streamed
+    assert np.array_equal(c3c, c3)
