@@ -288,16 +288,6 @@ k_segsort(const OffT *__restrict__ seg, int64_t seg_lo, int64_t seg_hi, int64_t 
 }
 
 // ---- A2 / A4: neighbour count and fill ------------------------------------------------------------------
-__device__ __forceinline__ double sep1(double a, double b, int c)
-{   // separation component from a to b, minimum image when periodic (A-4)
-    double d = __dsub_rn(b, a);
-    if (c_bp.periodic) {
-        if (d > c_bp.half[c]) d = __dsub_rn(d, c_bp.box[c]);
-        else if (d < -c_bp.half[c]) d = __dadd_rn(d, c_bp.box[c]);
-    }
-    return d;
-}
-
 __device__ __forceinline__ int bin_of(double d2)
 {   // b = #{k in [1,nb): q_k <= d2} (A-3); q is non-decreasing so this is an upper bound search
     int lo = 1, hi = c_bp.nb;            // answer = (first k in [1,nb) with q_k > d2) - 1
@@ -373,41 +363,83 @@ k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const
     int64_t out = 0;
     if (FILL) out = ptr[li] - e0;
     int count = 0;
-    for (int r = 0; r < ncell; ++r) {
-        const int src = __ffs(__ballot_sync(0xffffffffu, keep && rank == r)) - 1;
-        int b = __shfl_sync(0xffffffffu, cs, src);
-        const int e = __shfl_sync(0xffffffffu, ce, src);
-        const int cid = __shfl_sync(0xffffffffu, id, src);
-        if (c_bp.spatial && cid == own) b = (int)s + 1;
-        for (int t0 = b; t0 < e; t0 += 32) {
+    // The (cell, 32-candidate chunk) pairs are walked as one sequence with the NEXT chunk's label and
+    // coordinates already in flight while the current chunk's distances are evaluated (a cell holds about one
+    // chunk in the 1e6-point configurations, so without this every chunk pays the full load latency).
+    int r = -1, t0 = -32, e = -32;             // last consumed cell rank, chunk start, range end (warp-uniform)
+    // Cells adjacent in x have adjacent slot ranges, so a partial chunk at the end of one cell is topped up from
+    // the next cell when that one starts where this one ends (a cell holds ~28 points in the 1e6-point
+    // configurations: 18 chunks per point without this, ~13 with).
+    auto advance = [&]() -> bool {             // move to the next non-empty chunk; false when the stencil is done
+        t0 += 32;
+        for (;;) {
+            if (t0 + 32 <= e) return true;                     // a full chunk is left in the current range
+            if (r + 1 >= ncell) return t0 < e;
+            const int src = __ffs(__ballot_sync(0xffffffffu, keep && rank == r + 1)) - 1;
+            int b2 = __shfl_sync(0xffffffffu, cs, src);
+            const int e2 = __shfl_sync(0xffffffffu, ce, src);
+            const int cid = __shfl_sync(0xffffffffu, id, src);
+            if (c_bp.spatial && cid == own) b2 = (int)s + 1;
+            if (t0 >= e) { ++r; t0 = b2; e = e2; continue; }    // range exhausted: jump to the next cell
+            if (b2 == e) { ++r; e = e2; continue; }             // next cell is contiguous: extend the range
+            return true;                                       // partial chunk, next cell elsewhere
+        }
+    };
+    // loop invariants out of constant memory (the compiler re-issued ~13 constant loads per chunk)
+    const bool per = c_bp.periodic != 0;
+    const double hx = per ? c_bp.half[0] : INFINITY, hy = per ? c_bp.half[1] : INFINITY, hz = per ? c_bp.half[2] : INFINITY;
+    const double bx = c_bp.box[0], by = c_bp.box[1], bz = c_bp.box[2];
+    const double q_lo = c_q[0], q_hi = c_q[c_bp.nb];
+    // separation component a -> b, minimum image when periodic (A-4); half = +inf switches the wrap off
+    auto sep = [](double a, double b, double half, double box) -> double {
+        double d = __dsub_rn(b, a);
+        if (d > half) d = __dsub_rn(d, box);
+        else if (d < -half) d = __dadd_rn(d, box);
+        return d;
+    };
+    bool have = advance();
+    int n_lj = 0;
+    double n_x = 0.0, n_y = 0.0, n_z = 0.0;
+    bool n_ok = false;
+    if (have) {
+        const int t = t0 + lane;
+        n_ok = t < e;
+        if (n_ok) { n_lj = lab[t]; n_x = sx[t]; n_y = sy[t]; n_z = sz[t]; }
+    }
+    while (have) {
+        const bool ok = n_ok;
+        const int lj = n_lj;
+        const double xj = n_x, yj = n_y, zj = n_z;
+        have = advance();
+        n_ok = false;
+        if (have) {
             const int t = t0 + lane;
-            bool edge = false;
-            int lj = 0, bb = 0, pp = 0;
-            if (t < e) {
-                lj = lab[t];
-                if (lj > li) {
-                    // direction lower label -> higher label (hub -> spoke)
-                    const double dx = sep1(xi, sx[t], 0), dy = sep1(yi, sy[t], 1), dz = sep1(zi, sz[t], 2);
-                    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-                    edge = (d2 >= c_q[0]) && (d2 < c_q[c_bp.nb]);      // r_min <= r < r_max (A-2)
-                    if (FILL && edge) {
-                        bb = bin_of(d2);
-                        if (c_bp.want_pix) pp = pixel_of(dx, dy, dz, d2);
-                    }
-                }
+            n_ok = t < e;
+            if (n_ok) { n_lj = lab[t]; n_x = sx[t]; n_y = sy[t]; n_z = sz[t]; }
+        }
+        bool edge = false;
+        int bb = 0, pp = 0;
+        if (ok && lj > li) {
+            // direction lower label -> higher label (hub -> spoke)
+            const double dx = sep(xi, xj, hx, bx), dy = sep(yi, yj, hy, by), dz = sep(zi, zj, hz, bz);
+            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            edge = (d2 >= q_lo) && (d2 < q_hi);                // r_min <= r < r_max (A-2)
+            if (FILL && edge) {
+                bb = bin_of(d2);
+                if (c_bp.want_pix) pp = pixel_of(dx, dy, dz, d2);
             }
-            const unsigned m = __ballot_sync(0xffffffffu, edge);
-            if (FILL) {
-                if (edge) {
-                    const int64_t o = out + __popc(m & ((1u << lane) - 1u));
-                    idx[o] = lj;
-                    bin[o] = (uint8_t)bb;
-                    if (pix) pix[o] = (uint8_t)pp;
-                }
-                out += __popc(m);
-            } else {
-                count += __popc(m);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, edge);
+        if (FILL) {
+            if (edge) {
+                const int64_t o = out + __popc(m & ((1u << lane) - 1u));
+                idx[o] = lj;
+                bin[o] = (uint8_t)bb;
+                if (pix) pix[o] = (uint8_t)pp;
             }
+            out += __popc(m);
+        } else {
+            count += __popc(m);
         }
     }
     if (!FILL && lane == 0) deg[li] = count;
