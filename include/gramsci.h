@@ -55,7 +55,7 @@ typedef enum {
 /* 3pCF intersection kernel variants (S:8(f) rank 2 ablation). 0 picks the default. */
 enum {
     GRAMSCI_ALGO_DEFAULT = 0,
-    GRAMSCI_ALGO_MERGEPATH = 1, /* merge-path partitioned two-list intersection (P:57-70 on a warp) */
+    GRAMSCI_ALGO_MERGEPATH = 1, /* merge-path partitioned two-pointer walk (P:57-70 on a warp), hub row staged by TMA */
     GRAMSCI_ALGO_BSEARCH = 2,   /* lane-parallel binary search of N+(j) in the hub tail */
     GRAMSCI_ALGO_BITMAP = 3,    /* hub row scattered into a shared-memory slot table, O(1) membership;
                                    the default when the table fits (labels in cell order)               */

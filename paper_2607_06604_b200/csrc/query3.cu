@@ -149,6 +149,182 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
     }
 }
 
+// ---- 3pCF, merge-path variant (the paper's two-pointer walk, partitioned over a warp) ----------------
+// BASELINE's sketch of the kernel: a warp takes a hub-spoke pair and intersects the hub tail (shared memory) with
+// the spoke row N+(j) by a merge: the row is staged through a per-warp shared buffer in tiles, the part of the
+// tail a tile can meet is located with a 32-ary search, the merged sequence of the two pieces is cut into 32
+// equal diagonals (one binary search per lane on its diagonal), and every lane walks its piece with the
+// two-pointer rule of P:59-70 -- on a tie the row element is consumed first, and a row element is a hit iff the
+// current head of the tail equals it, so each triangle is found by exactly one lane.
+// The hub row itself arrives by one TMA bulk copy per array (cp.async.bulk -> UBLKCP, mbarrier completion).
+// Kept as GRAMSCI_ALGO_MERGEPATH for the ablation DESIGN.md section 6 reports; the slot table beats it.
+constexpr int MP_TILE = 512;          // row elements staged per warp and tile
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
+                 "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(dst)),
+                 "l"(src), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+
+template <bool WEIGHTED>
+__global__ void __launch_bounds__(Q3_THREADS)
+k_3pcf_merge(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
+             unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    // layout: [w row_cap*8 (W)] [idx raw (row_cap+8)*4] [bin raw row_cap+32] [hist nh*4] [per warp: tile idx, tile bin]
+    double *a_w = (double *)smem;
+    int32_t *raw_idx = (int32_t *)(smem + (WEIGHTED ? (size_t)p.row_cap * 8 : 0));
+    uint8_t *raw_bin = (uint8_t *)(raw_idx + p.row_cap + 8);
+    uint32_t *hist = (uint32_t *)(raw_bin + p.row_cap + 32);
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    int32_t *t_idx = (int32_t *)(hist + p.nh) + warp * MP_TILE;
+    uint8_t *t_bin = (uint8_t *)((int32_t *)(hist + p.nh) + Q3_WARPS * MP_TILE) + warp * MP_TILE;
+    __shared__ int s_slot;
+    __shared__ __align__(8) uint64_t s_bar;
+    unsigned long long budget = 0;
+    unsigned phase = 0;
+
+    const int nb = p.nb;
+    for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) hist[t] = 0;
+    if (threadIdx.x == 0) {
+        mbar_init(&s_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    double *my_w = WEIGHTED ? g_w + (size_t)blockIdx.x * p.nh : nullptr;
+    __syncthreads();
+
+    for (;;) {
+        if (threadIdx.x == 0) s_slot = v.s_lo + (int)atomicAdd(hub_counter, 1u);
+        __syncthreads();
+        const int s = s_slot;
+        if (s >= v.s_hi) break;
+        const int32_t i = v.order[s];
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
+        const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
+        const int n = (int)(re - rb);
+        if (n >= 2) {
+            if (budget + (unsigned long long)n * (n - 1) / 2 > 0xF0000000ull) {      // uint32 bins cannot wrap
+                for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) {
+                    const uint32_t c = hist[t];
+                    if (c) { atomicAdd(&g_cnt[t], (unsigned long long)c); hist[t] = 0; }
+                }
+                budget = 0;
+            }
+            budget += (unsigned long long)n * (n - 1) / 2;
+            // ---- hub row by TMA: bulk copies need 16-byte aligned source, destination and size, so each array is
+            // copied from its address rounded down and used at the matching offset
+            const int32_t *gi = v.idx_h + (rb - v.e0_h);
+            const uint8_t *gb = v.bin_h + (rb - v.e0_h);
+            const unsigned xi = (unsigned)(((uintptr_t)gi & 15) >> 2), xb = (unsigned)((uintptr_t)gb & 15);
+            const unsigned bytes_i = (((unsigned)n + xi) * 4 + 15) & ~15u, bytes_b = ((unsigned)n + xb + 15) & ~15u;
+            if (threadIdx.x == 0) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // earlier generic reads of the row buffers
+                mbar_expect_tx(&s_bar, bytes_i + bytes_b);
+                tma_bulk_g2s(raw_idx, (const void *)((uintptr_t)gi & ~(uintptr_t)15), bytes_i, &s_bar);
+                tma_bulk_g2s(raw_bin, (const void *)((uintptr_t)gb & ~(uintptr_t)15), bytes_b, &s_bar);
+            }
+            const int32_t *a_idx = raw_idx + xi;
+            const uint8_t *a_bin = raw_bin + xb;
+            if (WEIGHTED)
+                for (int t = threadIdx.x; t < n; t += Q3_THREADS) a_w[t] = v.w[gi[t]];
+            mbar_wait(&s_bar, phase);
+            phase ^= 1;
+            __syncthreads();
+
+            const double wi = WEIGHTED ? v.w[i] : 1.0;
+            for (int a = warp; a < n - 1; a += Q3_WARPS) {
+                const int32_t j = a_idx[a];
+                if (j < v.c_lo || j >= v.c_hi) continue;          // foreign spoke
+                const int64_t jb = v.ptr[j];
+                const int nj = (int)(v.ptr[j + 1] - jb);
+                const int32_t *B = v.idx_c + (jb - v.e0_c);
+                const uint8_t *Bb = v.bin_c + (jb - v.e0_c);
+                const int32_t *A = a_idx + a + 1;                 // hub tail {k in N+(i): k > j}
+                const int nA = n - a - 1;
+                const int32_t a_last = A[nA - 1];
+                const int hbase = (int)a_bin[a] * nb * nb;
+                const double wij = WEIGHTED ? wi * a_w[a] : 1.0;
+                int alo = 0;                                      // tail elements below every later row element
+                for (int b0 = 0; b0 < nj && alo < nA; b0 += MP_TILE) {
+                    const int nB = min(MP_TILE, nj - b0);
+                    __syncwarp();
+                    for (int t = lane; t < nB; t += 32) { t_idx[t] = B[b0 + t]; t_bin[t] = Bb[b0 + t]; }
+                    __syncwarp();
+                    const int32_t b_first = t_idx[0], b_last = t_idx[nB - 1];
+                    // 32-ary searches: first tail element >= b_first, first tail element > b_last
+                    auto lower = [&](int32_t key, int lo) {        // first x in [lo,nA) with A[x] >= key (nA if none)
+                        int hi = nA;                               // candidates [lo,hi), answer in [lo,hi]
+                        while (hi > lo) {
+                            const int stride = (hi - lo + 31) >> 5;
+                            const int x = lo + (lane + 1) * stride - 1;          // 32 probes, the last ones may fall off
+                            const int c = __popc(__ballot_sync(0xffffffffu, x < hi && A[x] < key));   // a prefix of lanes
+                            hi = min(lo + (c + 1) * stride - 1, hi);   // probe c is >= key (or off the end)
+                            lo = lo + c * stride;                      // everything up to probe c-1 is < key
+                        }
+                        return lo;
+                    };
+                    alo = lower(b_first, alo);
+                    const int ahi = (b_last >= a_last) ? nA : lower(b_last + 1, alo);
+                    const int nAt = ahi - alo;
+                    if (nAt > 0) {
+                        // merge path: diagonal d = lane * L of the (nAt + nB)-long merged sequence
+                        const int T = nAt + nB, L = (T + 31) >> 5;
+                        const int d0 = min(lane * L, T), d1 = min(d0 + L, T);
+                        int lo = max(0, d0 - nB), hi = min(d0, nAt);
+                        while (lo < hi) {                              // ties: the row element goes first
+                            const int mid = (lo + hi) >> 1;
+                            if (A[alo + mid] < t_idx[d0 - 1 - mid]) lo = mid + 1; else hi = mid;
+                        }
+                        int ia = lo, ib = d0 - lo;
+                        for (int step = d0; step < d1; ++step) {
+                            const int32_t av = (ia < nAt) ? A[alo + ia] : INT32_MAX;
+                            const int32_t bv = (ib < nB) ? t_idx[ib] : INT32_MAX;
+                            if (ib < nB && bv <= av) {
+                                if (bv == av) {
+                                    const int pos = a + 1 + alo + ia;
+                                    const int h = hbase + (int)a_bin[pos] * nb + (int)t_bin[ib];
+                                    if (p.want_counts) atomicAdd(&hist[h], 1u);
+                                    if (WEIGHTED) atomicAdd(&my_w[h], wij * a_w[pos]);
+                                }
+                                ++ib;
+                            } else {
+                                ++ia;
+                            }
+                        }
+                    }
+                    alo = ahi;
+                    if (b_last >= a_last) break;                    // the tail is used up
+                }
+            }
+        }
+        __syncthreads();
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) {
+        const uint32_t c = hist[t];
+        if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
+    }
+}
+
 // ---- 3pCF, slot-table variant (default) ------------------------------------------------------------------
 // Membership of k in N+(i) is one table lookup instead of a search (the hub-side analogue of the paper's
 // lmat idea: spend O(len) setup per hub to make every later test O(1)).  The hub row is scattered
@@ -519,7 +695,7 @@ struct Q3Run {
     double *raw_w;
     int grid;
     size_t smem;
-    int use_table, G, long_rows;
+    int use_table, G, long_rows, use_merge;
 };
 
 template <bool W, int U>
@@ -548,7 +724,10 @@ void tile_3pcf(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
 {
     Q3Run *r = (Q3Run *)user;
     GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
-    if (r->use_table) {
+    if (r->use_merge) {
+        if (r->p.weighted) k_3pcf_merge<true><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
+        else k_3pcf_merge<false><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
+    } else if (r->use_table) {
         if (r->p.weighted) { if (r->long_rows) launch_table<true, 8>(r, v, st); else launch_table<true, 4>(r, v, st); }
         else { if (r->long_rows) launch_table<false, 8>(r, v, st); else launch_table<false, 4>(r, v, st); }
     } else if (r->p.weighted)
@@ -621,7 +800,8 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     r.G = 8;
     // rows of hundreds of entries and more stream from DRAM (the CSR no longer lives in L2): keep 8 windows in flight
     r.long_rows = (g->n > 0 && g->n_edges / g->n >= 512) ? 1 : 0;
-    if (g->algo != GRAMSCI_ALGO_BSEARCH && g->max_row >= 2 && g->max_row < 65535) {
+    r.use_merge = (g->algo == GRAMSCI_ALGO_MERGEPATH) ? 1 : 0;
+    if (g->algo != GRAMSCI_ALGO_BSEARCH && !r.use_merge && g->max_row >= 2 && g->max_row < 65535) {
         const size_t hist_bytes = (((size_t)nh * 4 + 15) & ~(size_t)15) + 16;
         int best_s = -1, ptl = 0, tbl = 0;
         size_t best = 0;
@@ -653,7 +833,13 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table does not fit in shared memory (longest row %d)", g->max_row);
     }
     const void *fn;
-    if (r.use_table) {
+    if (r.use_merge) {
+        const size_t rc = (size_t)r.p.row_cap;
+        r.smem = (W ? rc * 8 : 0) + (rc + 8) * 4 + rc + 32 + (size_t)nh * 4 + (size_t)Q3_WARPS * MP_TILE * 5 + 64;
+        if (r.smem > g->smem_optin)
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
+        fn = W ? (const void *)k_3pcf_merge<true> : (const void *)k_3pcf_merge<false>;
+    } else if (r.use_table) {
         fn = W ? (r.long_rows ? table_fn<true, 8>(r.G) : table_fn<true, 4>(r.G))
                : (r.long_rows ? table_fn<false, 8>(r.G) : table_fn<false, 4>(r.G));
     } else {

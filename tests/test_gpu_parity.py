@@ -75,7 +75,7 @@ def test_2pcf(relabel):
     assert_weighted_close(w, ow)
 
 
-ALGOS = [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G1, gr.ALGO_TABLE_G2, gr.ALGO_TABLE_G4, gr.ALGO_TABLE_G8]
+ALGOS = [gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G1, gr.ALGO_TABLE_G2, gr.ALGO_TABLE_G4, gr.ALGO_TABLE_G8]
 
 
 @pytest.mark.parametrize("algo", ALGOS)
@@ -222,7 +222,7 @@ def test_4pcf_edge_cases():
 
 
 # ---- larger / clustered shapes and the out-of-core tiler (S:8(a) A11; pin C-13) -----------------------------
-@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4])
+@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4])
 def test_3pcf_clustered_replica(algo):
     """1/64 replica of BASELINE configs[1] data (Neyman-Scott, same densities, fp64 weights)."""
     cfg = cat.config2_data(seed=2101, n=15_625, L=250.0, mean_parents=156.25)
@@ -245,7 +245,7 @@ def _bao_replica():
     return _BAO["cfg"], _BAO["cnt"]
 
 
-@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G8])
+@pytest.mark.parametrize("algo", [gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G8])
 def test_3pcf_bao_replica(algo):
     """Shrunk replica of BASELINE configs[4] (same radii and bins, L=310, 40 % of the density so that
     the oracle finishes in seconds): rows of thousands of entries, r_min > 0, 18 bins, a periodic grid
@@ -379,7 +379,7 @@ def test_full_size_config4_parity_sampled_hubs():
 def test_hub_stride_partial_results():
     cfg = small(41, n=3000, L=30.0, weighted=True, r_max=5.0, nb=4)
     og = oracle.Graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
-    for algo in (gr.ALGO_DEFAULT, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4):
+    for algo in (gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G4):
         g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
                                    relabel=2, hub_stride=7, algo=algo)
         assert np.array_equal(g.pcf3()[0], og.pcf3(hubs=(0, og.n, 7))[0])
