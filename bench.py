@@ -349,7 +349,9 @@ def run_ours(args):
     else:
         # 4pCF kernels are bound by the L2 atomic rate: one RED per hit and output channel;
         # peak = RED.E.ADD.64 rate measured on this pool's B200 by csrc/ubench_atomics.cu (profiles/r1_ubench_atomics.txt)
-        ch = 1 if cats[dom]["weights"] is None else (4 if kind0 == "4pcf_parity" else 2)
+        # one RED per hit and kind of output (counts, weighted sums); the parity split costs no extra RED: a hit goes
+        # to the raw histogram of its sign class and the fold forms even / odd
+        ch = 1 if cats[dom]["weights"] is None else 2
         red_rate = dw["hits"] * ch / dom_s / 1e9
         roof = {"bound": "l2-atomics", "achieved": red_rate, "peak": RED_PEAK_GOPS, "unit": "Gatomic/s",
                 "frac": red_rate / RED_PEAK_GOPS, "traffic": None, "kernel": f"{kern} on {dw['name']}",

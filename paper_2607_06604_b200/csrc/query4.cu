@@ -17,9 +17,11 @@
 //            streamed the byte rows; with rows of ~50 entries most lanes idled: 37 ms vs now on cfg3.)
 //
 // Parity (Eq. 3; A-8..A-11): V = (n_a x n_b) . n_c on the pixel-centre unit vectors of the three
-// hub spokes, every product and sum rounded separately; the kernel accumulates sign(V) (0 when
-// |V| < 1e-9) per RAW tuple and the fold applies the chirality factor of the raw tuple, which for the
-// raw tuple t^sigma of a canonical chiral tuple t is sgn(sigma) (and 0 for bin-achiral t).
+// hub spokes, every product and sum rounded separately; the kernel files every hit under the RAW tuple in
+// one of three sign classes (V > 0, V < 0, |V| < 1e-9) -- one atomic per hit and kind of output instead of
+// separate even and odd updates -- and the fold forms even = pos + neg + degenerate and odd = chi (pos - neg)
+// with the chirality factor of the raw tuple, which for the raw tuple t^sigma of a canonical chiral tuple t
+// is sgn(sigma) (and 0 for bin-achiral t).
 //
 // D lives in shared memory when the longest row allows (a few hundred entries), else in a per-CTA slice of a
 // global scratch (the paper's "per-gang slice of a global scratch sized from the longest row"),
@@ -108,11 +110,10 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         if (w_o) w_o += (size_t)blockIdx.x * p.ncfg;
         for (int t = threadIdx.x; t < ncfg_pad; t += Q4_THREADS) h_e[t] = 0u;
     } else {
-        const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh;
+        // raw mode: [n_shards][nh], or [n_shards][3][nh] (sign classes) for the parity split
+        const size_t shard = (size_t)(blockIdx.x % p.n_shards) * (size_t)p.nh * (p.parity ? 3 : 1);
         if (cnt_e) cnt_e += shard;
-        if (cnt_o) cnt_o += shard;
         if (w_e) w_e += shard;
-        if (w_o) w_o += shard;
     }
     if (p.parity)
         for (int t = threadIdx.x; t < 256 * 3; t += Q4_THREADS) s_tab[t] = pix_tab[t];
@@ -219,13 +220,15 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
                             if (cnt_o) atomicAdd(&h_o[cid], sg);
                             if (w_o) atomicAdd(&w_o[cid], sg > 0 ? ww : -ww);
                         }
+                    } else if (p.parity) {
+                        // one RED per hit and kind of output: the hit goes to the class of its sign (V > 0, V < 0,
+                        // degenerate); even = sum of the classes, odd = pos - neg, formed by the fold
+                        const size_t y = (size_t)(sg > 0 ? 0 : (sg < 0 ? 1 : 2)) * (size_t)p.nh + x;
+                        if (cnt_e) atomicAdd(&cnt_e[y], 1ull);
+                        if (p.weighted) atomicAdd(&w_e[y], ww);
                     } else {
                         if (cnt_e) atomicAdd(&cnt_e[x], 1ull);
                         if (p.weighted) atomicAdd(&w_e[x], ww);
-                        if (sg != 0) {
-                            if (cnt_o) atomicAdd(&cnt_o[x], sg > 0 ? 1ull : ~0ull);     // += +-1 (mod 2^64)
-                            if (w_o) atomicAdd(&w_o[x], sg > 0 ? ww : -ww);
-                        }
                     }
                 }
             }
@@ -355,7 +358,7 @@ __global__ void k_fold4_cfg(int ncfg, int n_slabs, const int32_t *__restrict__ d
 }
 
 // ---- A10 fold: raw 6-tuples -> canonical configurations (A-7), odd channel with the chirality sign (A-10) ---
-__global__ void k_fold4(int nb, int64_t nh, int n_shards, const unsigned long long *__restrict__ cnt_e,
+__global__ void k_fold4(int nb, int64_t nh, int n_shards, int cls3, const unsigned long long *__restrict__ cnt_e,
                         const unsigned long long *__restrict__ cnt_o, const double *__restrict__ w_e,
                         const double *__restrict__ w_o, unsigned long long *__restrict__ out_ce,
                         long long *__restrict__ out_co, double *__restrict__ out_we, double *__restrict__ out_wo)
@@ -399,12 +402,22 @@ __global__ void k_fold4(int nb, int64_t nh, int n_shards, const unsigned long lo
                 for (int b = a + 1; b < 4; ++b) inv += (q[a] > q[b]) ? 1 : 0;
             const int sg = (inv & 1) ? -1 : 1;
             for (int sh = 0; sh < n_shards; ++sh) {
-                const size_t y = (size_t)sh * (size_t)nh + (size_t)ys[s];
-                if (cnt_e) ce += cnt_e[y];
-                if (w_e) we += w_e[y];
-                if (!odd_aut) {
-                    if (cnt_o) co += (long long)sg * (long long)cnt_o[y];
-                    if (w_o) wo += (double)sg * w_o[y];
+                if (cls3) {            // parity: raw classes pos / neg / degenerate per shard
+                    const size_t y = (size_t)sh * 3 * (size_t)nh + (size_t)ys[s];
+                    if (cnt_e) {
+                        const unsigned long long cp = cnt_e[y], cn = cnt_e[y + nh], cz = cnt_e[y + 2 * nh];
+                        ce += cp + cn + cz;
+                        if (!odd_aut) co += (long long)sg * ((long long)cp - (long long)cn);
+                    }
+                    if (w_e) {
+                        const double wp = w_e[y], wn = w_e[y + nh], wz = w_e[y + 2 * nh];
+                        we += (wp + wn) + wz;
+                        if (!odd_aut) wo += (double)sg * (wp - wn);
+                    }
+                } else {
+                    const size_t y = (size_t)sh * (size_t)nh + (size_t)ys[s];
+                    if (cnt_e) ce += cnt_e[y];
+                    if (w_e) we += w_e[y];
                 }
             }
         }
@@ -437,7 +450,11 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     p.row_cap = std::max(16, (g->max_row + 15) & ~15);
     const int channels = (d_even_c ? 1 : 0) + (d_odd_c ? 1 : 0) + (d_even_w ? 1 : 0) + (d_odd_w ? 1 : 0);
     if (channels == 0) { GR_CUDA(cudaStreamSynchronize(st)); g->t_query_ms = total.stop(); return; }
-    p.n_shards = (int)std::max<int64_t>(1, std::min<int64_t>(8, ((int64_t)64 << 20) / (nh * 8 * channels)));
+    {   // raw histograms kept per launch: counts and/or weights, three sign classes each for the parity split
+        const int kinds = ((d_even_c || d_odd_c) ? 1 : 0) + ((d_even_w || d_odd_w) ? 1 : 0);
+        const int64_t per_shard = nh * 8 * kinds * (p.parity ? 3 : 1);
+        p.n_shards = (int)std::max<int64_t>(1, std::min<int64_t>(8, ((int64_t)96 << 20) / per_shard));
+    }
 
     const size_t rc = (size_t)p.row_cap;
     if (rc >= 65536) GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) exceeds 65535", g->max_row);
@@ -495,12 +512,13 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     counter.alloc(1);
     GR_CUDA(cudaMemsetAsync(counter.p, 0, sizeof(unsigned int), st));
     // LUT: counts [ncfg], weights [grid][ncfg]; raw: [n_shards][nh] each
-    const size_t tot_c = use_lut ? (size_t)p.ncfg : (size_t)nh * p.n_shards;
-    const size_t tot_w = use_lut ? (size_t)p.ncfg * grid : (size_t)nh * p.n_shards;
-    if (d_even_c) { ce.alloc(tot_c); GR_CUDA(cudaMemsetAsync(ce.p, 0, tot_c * 8, st)); }
-    if (d_odd_c) { co.alloc(tot_c); GR_CUDA(cudaMemsetAsync(co.p, 0, tot_c * 8, st)); }
+    const size_t raw = (size_t)nh * p.n_shards * (p.parity ? 3 : 1);
+    const size_t tot_c = use_lut ? (size_t)p.ncfg : raw;
+    const size_t tot_w = use_lut ? (size_t)p.ncfg * grid : raw;
+    if (d_even_c || (!use_lut && d_odd_c)) { ce.alloc(tot_c); GR_CUDA(cudaMemsetAsync(ce.p, 0, tot_c * 8, st)); }
+    if (use_lut && d_odd_c) { co.alloc(tot_c); GR_CUDA(cudaMemsetAsync(co.p, 0, tot_c * 8, st)); }
     if (d_even_w || d_odd_w) { we.alloc(tot_w); GR_CUDA(cudaMemsetAsync(we.p, 0, tot_w * 8, st)); }
-    if (d_odd_w) { wo.alloc(tot_w); GR_CUDA(cudaMemsetAsync(wo.p, 0, tot_w * 8, st)); }
+    if (use_lut && d_odd_w) { wo.alloc(tot_w); GR_CUDA(cudaMemsetAsync(wo.p, 0, tot_w * 8, st)); }
     if (p.parity) {
         // pixel-centre unit vectors (A-8): z_c = (iz + 1/2)/8 - 1, phi_c = (iphi + 1/2) pi/8
         std::vector<double> h(256 * 3);
@@ -551,7 +569,7 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
                                                          d_odd_w ? wo.p : nullptr, (unsigned long long *)d_even_c,
                                                          (long long *)d_odd_c, d_even_w, d_odd_w);
     } else {
-        k_fold4<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, p.n_shards, ce.p, co.p, d_even_w ? we.p : nullptr, wo.p,
+        k_fold4<<<(unsigned)((nh + 127) / 128), 128, 0, st>>>(nb, nh, p.n_shards, p.parity, ce.p, co.p, we.p, wo.p,
                                                               (unsigned long long *)d_even_c, (long long *)d_odd_c,
                                                               d_even_w, d_odd_w);
     }
