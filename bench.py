@@ -393,7 +393,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--algo", type=int, default=0)
-    ap.add_argument("--ref-stride", type=int, default=8)
+    ap.add_argument("--ref-stride", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-4pcf", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true", help="big workloads only: no host-buffer leg (e2e = null)")
