@@ -38,6 +38,7 @@ DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 577.233152e6 + 5.401344e6,
                       "k_3pcf_table<counts>": 302.012672e6 + 4.176896e6}
 
 
+L2_READ_GBS = 12000.0      # L2 -> SM read bandwidth, 16-byte loads over a 32-64 MB working set (same micro-benchmark)
 RED_PEAK_GOPS = 193.0      # global RED.E.ADD.(U64|F64), spread addresses, all SMs: best line of the micro-benchmark,
                            # whose loop overhead makes it a slight under-estimate (kernels reach ~1.1 of it)
 
@@ -342,6 +343,14 @@ def run_ours(args):
                 "launch_ms": enum_ms[dom], "algorithmic_bytes_per_launch": dw["bytes"],
                 "units_per_launch": {"spoke_row_elements": dw["spoke"], "tail_elements": dw["tail"],
                                      "hub_spoke_pairs": dw["edges"], "hits": dw["hits"]},
+                # t_roof = max(CSR once from HBM, spoke rows + hit bytes from L2); fraction = t_roof / t
+                "l2_roofline": {"l2_peak_gbs": L2_READ_GBS,
+                                "t_roof_ms": 1e3 * max(5.0 * dw["edges"] / (peak * 1e9),
+                                                       (4.0 * dw["spoke"] + dw["hits"]) / (L2_READ_GBS * 1e9)),
+                                "frac": max(5.0 * dw["edges"] / (peak * 1e9),
+                                            (4.0 * dw["spoke"] + dw["hits"]) / (L2_READ_GBS * 1e9)) / dom_s},
+                "per_launch": [{"catalogue": w_["name"], "launch_ms": enum_ms[k_], "achieved": w_["bytes"] / (enum_ms[k_] * 1e-3) / 1e9,
+                                "frac": w_["bytes"] / (enum_ms[k_] * 1e-3) / 1e9 / peak} for k_, w_ in enumerate(work)],
                 "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits (DESIGN.md "
                         "section 6); spoke rows are re-read from L2/L1, so this is an L2->SM figure and may "
                         "exceed the HBM peak; traffic = dram read+write of one ncu --set full launch "

@@ -41,6 +41,23 @@ __global__ void k(int iters, int nbins, int active, unsigned long long *g64, dou
     __syncthreads();
     if(MODE<=2 && threadIdx.x==0) sink[1]+=h32[0];
 }
+// L2 -> SM read bandwidth: every CTA streams the whole working set (<= 64 MB, L2 resident after the first pass)
+// with 16-byte loads; DESIGN.md section 6 quotes it next to the HBM copy figure
+__global__ void k_l2read(const int4 *__restrict__ buf, size_t n16, int reps, int *sink)
+{
+    int acc = 0;
+    for (int r = 0; r < reps; ++r) {
+        const size_t off = ((size_t)r * 250112) % n16;        // a different rotation per pass: nothing to hoist
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) {
+            size_t j = i + off;
+            if (j >= n16) j -= n16;
+            const int4 v = __ldcg(buf + j);
+            acc += v.x ^ v.y ^ v.z ^ v.w;
+        }
+    }
+    if (acc == 0x7fffffff) sink[0] = acc;
+}
+
 template<int MODE> int run(const char*name,int nbins,int active,size_t smem,int ctas_per_sm, unsigned long long*g64,double*gd,unsigned long long*sink)
 {
     int iters=4096; int grid=148*ctas_per_sm;
@@ -77,5 +94,21 @@ int main(){
       run<8>("smem LDS u32 random",4096,act,4096*8,4,g64,gd,sink);
     }
     run<7>("match_any",256,32,1024,4,g64,gd,sink);
+    for (size_t mb : {16, 32, 64}) {
+        const size_t n16 = mb * (1 << 20) / 16;
+        int4 *buf; int *sk;
+        CK(cudaMalloc(&buf, n16 * 16)); CK(cudaMemset(buf, 1, n16 * 16)); CK(cudaMalloc(&sk, 4));
+        const int reps = 200;
+        k_l2read<<<148 * 8, 256>>>(buf, n16, 2, sk);
+        CK(cudaDeviceSynchronize());
+        cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+        cudaEventRecord(a);
+        k_l2read<<<148 * 8, 256>>>(buf, n16, reps, sk);
+        cudaEventRecord(b); CK(cudaDeviceSynchronize());
+        float ms; cudaEventElapsedTime(&ms, a, b);
+        printf("L2 read, %zu MB working set, 16-byte loads: %.3f ms for %d passes -> %.0f GB/s\n", mb, ms, reps,
+               (double)n16 * 16 * reps / (ms * 1e-3) / 1e9);
+        cudaFree(buf); cudaFree(sk);
+    }
     return 0;
 }
