@@ -394,7 +394,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
     const int nb = p.nb, nb2 = nb * nb;
     const int sh = p.s;
     const unsigned pm = (1u << sh) - 1u;
-    const unsigned ptl1 = (unsigned)p.pt_len - 1u;       // sentinel page: always chunk 0 (all EMPTY)
+    const unsigned dmax = ((unsigned)p.pt_len - 1u) << sh;  // first key of the sentinel page: always chunk 0 (all EMPTY)
     const unsigned lt_mask = (1u << lane) - 1u, le_mask = (2u << lane) - 1u;
     unsigned long long budget = 0;       // upper bound of the hits this warp added since it last flushed
     // key of a label k in the current hub's table: the largest gap of the row is cut out (rows next to a
@@ -490,7 +490,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
                 const bool np = ok && g != pg;
                 const unsigned m = __ballot_sync(0xffffffffu, np);
                 const int ch = cbase + __popc(m & le_mask);          // chunks are numbered from 1
-                if (np) pt[g] = (uint16_t)ch;
+                if (np) pt[g] = (uint16_t)((unsigned)ch << sh);      // slot base of the page's chunk
                 if (ok) tab[((unsigned)ch << sh) | (d & pm)] = WEIGHTED ? (slot_t)t : (slot_t)gb[t];
                 cbase += __popc(m);
                 carry = __shfl_sync(0xffffffffu, g, 31);
@@ -511,9 +511,9 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
         // the current row is looked up (rows are tens of entries long in the 1e6-point configurations)
         auto lookup = [&](int32_t k, unsigned gam, int hb, double wia) {
             const bool hi = k >= brk;
-            const unsigned d = min((unsigned)(k - (hi ? sub_hi : base)), hi ? 0xffffffffu : guard);
-            const unsigned ch = pt[min(d >> sh, ptl1)];
-            const unsigned e = tab[(ch << sh) | (d & pm)];
+            // one clamp does both ends: below / inside the gap -> guard page, beyond the row -> sentinel page
+            const unsigned d = min((unsigned)(k - (hi ? sub_hi : base)), hi ? dmax : guard);
+            const unsigned e = tab[(unsigned)pt[d >> sh] | (d & pm)];      // pt holds the slot base, chunk << s
             if (e != EMPTY) {
                 if (WEIGHTED) {
                     const int h = hb + (int)a_bin[e] * nb + (int)gam;
@@ -744,7 +744,7 @@ size_t table_group_bytes(const gramsci_graph *g, int s, bool weighted, int G, in
     const size_t a16 = 15;
     const int64_t ptl = (int64_t)g->max_ptl[s] + 1;      // + sentinel page
     const int64_t tbl = ((int64_t)g->max_pages[s] + 1) << s;
-    if (ptl > (1 << 20) || tbl > (1 << 20) || g->max_pages[s] >= 65535) return 0;
+    if (ptl > (1 << 20) || tbl > 65536 || g->max_pages[s] >= 65535) return 0;      // slot bases are uint16
     *pt_len = (int)ptl;
     *tab_len = (int)tbl;
     size_t b = (size_t)G * 32 * (16 + (weighted ? 8 : 0));
