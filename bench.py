@@ -121,6 +121,20 @@ def sum_over_ranks(value: float, device=None) -> float:
     return float(t.item())
 
 
+def allreduce_hist(arr, device=None):
+    """Strong-scaling mode: every rank enumerates the hubs of its shard of ONE catalogue (shard_count = world,
+    shard_index = rank); the histograms add up to the full result with one all-reduce (SUM) -- the only
+    collective a multi-GPU run of this path needs."""
+    import torch
+    import torch.distributed as dist
+    t = torch.from_numpy(np.ascontiguousarray(arr))
+    if device is not None:
+        t = t.to(device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return t.cpu().numpy()
+
+
 def workload(name: str, seed_shift: int = 0):
     """List of catalogues (dicts from catalogues.py) making up one batch."""
     if name == "cfg2":
@@ -214,7 +228,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gr.load_library()
 
-    cats = workload(args.workload, seed_shift=rank_seed_shift(rank))
+    strong = args.scaling == "strong" and world > 1
+    cats = workload(args.workload, seed_shift=0 if strong else rank_seed_shift(rank))
     dev = [(torch.from_numpy(c["points"]).cuda(), None if c["weights"] is None else torch.from_numpy(c["weights"]).cuda())
            for c in cats]
     pin = [(torch.from_numpy(c["points"]).pin_memory(), None if c["weights"] is None else torch.from_numpy(c["weights"]).pin_memory())
@@ -233,7 +248,8 @@ def run_ours(args):
             kind = c["kind"]
             g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo,
                                        want_pixels=(kind == "4pcf_parity"),
-                                       device_mem_cap_bytes=int(args.cap_gib * 2 ** 30))
+                                       device_mem_cap_bytes=int(args.cap_gib * 2 ** 30),
+                                       shard_count=world if strong else 0, shard_index=rank if strong else 0)
             st["build_ms"] += g.timing(0)
             st["launches"] += g.timing(3)
             if kind == "3pcf":
@@ -242,6 +258,10 @@ def run_ours(args):
                 cnt, ws = g.pcf4(counts=True, weighted=(w is not None), host=host)
             else:
                 cnt, _, ws, _ = g.pcf4_parity(counts=True, weighted=(w is not None), host=host)
+            if strong:                     # partial histograms of the shards -> full result on every rank
+                cnt = allreduce_hist(cnt, "cuda")
+                if ws is not None:
+                    ws = allreduce_hist(ws, "cuda")
             digest.update(np.ascontiguousarray(cnt).tobytes())
             pc = {"name": c["name"], "enum_ms": g.timing(2), "weighted": w is not None}
             st["enum_ms"] += g.timing(2)
@@ -302,7 +322,7 @@ def run_ours(args):
     else:
         ms_e2e, tri2, _, _ = timed(True, max(1, args.steps // 2), 1)
         assert tri2 == tri
-    tri_all = sum_over_ranks(float(tri), "cuda")
+    tri_all = float(tri) if strong else sum_over_ranks(float(tri), "cuda")
 
     # second headline of BASELINE.json's metric: 4pCF quadruplets/s on configs[2] (query only, rank 0, untimed region)
     four = None
@@ -368,7 +388,8 @@ def run_ours(args):
     line = {
         "metric": metric, "value": tri_all / (ms * 1e-3), "unit": unit,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
         "config": {"workload": args.workload, "catalogues": [c["name"] for c in cats],
                    "n_points": [int(c["points"].shape[0]) for c in cats], "tuples_per_step": tri,
                    "counts_sha1": stats.get("sha1"), "cap_gib": args.cap_gib, "n_windows": stats.get("windows"),
@@ -405,6 +426,9 @@ def main():
     ap.add_argument("--ref-stride", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-4pcf", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own catalogues (default); strong = the hubs of ONE workload "
+                         "sharded over the ranks (every rank builds the whole graph), histograms all-reduced")
     ap.add_argument("--skip-e2e", action="store_true", help="big workloads only: no host-buffer leg (e2e = null)")
     ap.add_argument("--cap-gib", type=float, default=0.0,
                     help="device_mem_cap_bytes in GiB (0 = whole CSR resident); forces the out-of-core tiler")

@@ -81,6 +81,11 @@ typedef struct {       /* zero-initialised struct == defaults */
                                       == 0 (a sampled partial result, for checking full-size runs against a
                                       reference that is too slow to run in full); needs caller labels
                                       (relabel = 2 or want_pixels), else GRAMSCI_EINVAL                    */
+    int shard_count, shard_index;  /* shard_count > 1: this graph's queries enumerate only the tuples whose hub (the
+                                      vertex with the smallest internal label) has label % shard_count ==
+                                      shard_index.  The shards partition the tuples: the histograms of shards
+                                      0..shard_count-1 add up to the full result, exactly for counts -- one GPU
+                                      per shard and one all-reduce of the histogram (S:8(e)); 2pCF is not sharded */
 } gramsci_options;
 
 /*

@@ -43,7 +43,8 @@ class GramsciError(RuntimeError):
 class _Options(ctypes.Structure):
     _fields_ = [("stream", ctypes.c_void_p), ("device_mem_cap_bytes", ctypes.c_uint64),
                 ("want_pixels", ctypes.c_int), ("relabel", ctypes.c_int), ("algo", ctypes.c_int),
-                ("n_windows", ctypes.c_int), ("hub_stride", ctypes.c_int)]
+                ("n_windows", ctypes.c_int), ("hub_stride", ctypes.c_int),
+                ("shard_count", ctypes.c_int), ("shard_index", ctypes.c_int)]
 
 
 _lib = None
@@ -209,7 +210,8 @@ class Graph:
 
 def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = None, r_min: float = 0.0,
                         r_max: float = 1.0, nbins: int = 1, *, want_pixels: bool = False, relabel: int = 0,
-                        algo: int = 0, device_mem_cap_bytes: int = 0, n_windows: int = 0, hub_stride: int = 0) -> Graph:
+                        algo: int = 0, device_mem_cap_bytes: int = 0, n_windows: int = 0, hub_stride: int = 0,
+                        shard_count: int = 0, shard_index: int = 0) -> Graph:
     """``gramsci_build_graph`` (include/gramsci.h).  ``points`` [N,3] / ``weights`` [N] fp64: torch CUDA
     tensors (used in place), torch CPU tensors or NumPy arrays (the library stages host buffers itself)."""
     L = load_library()
@@ -234,6 +236,8 @@ def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = N
     opt.algo = int(algo)
     opt.n_windows = int(n_windows)
     opt.hub_stride = int(hub_stride)
+    opt.shard_count = int(shard_count)
+    opt.shard_index = int(shard_index)
     cbox = None
     if box is not None:
         cbox = (ctypes.c_double * 3)(*[float(v) for v in box])

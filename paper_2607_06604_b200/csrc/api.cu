@@ -171,7 +171,8 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     gramsci_options o;
     memset(&o, 0, sizeof o);
     if (opt) o = *opt;
-    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0 || o.hub_stride < 0)
+    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0 || o.hub_stride < 0 ||
+        o.shard_count < 0 || o.shard_index < 0 || (o.shard_count > 1 && o.shard_index >= o.shard_count))
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: bad options");
     require_device();
 
@@ -203,6 +204,8 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->spatial = (o.relabel == 1) ? 1 : (o.relabel == 2) ? 0 : (o.want_pixels ? 0 : 1);
     g->algo = o.algo;
     g->hub_stride = o.hub_stride > 1 ? o.hub_stride : 1;
+    g->shard_count = o.shard_count > 1 ? o.shard_count : 1;
+    g->shard_index = o.shard_count > 1 ? o.shard_index : 0;
     if (g->hub_stride > 1 && g->spatial) {
         delete g; g = nullptr;
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: hub_stride needs caller labels (relabel = 2 or want_pixels)");

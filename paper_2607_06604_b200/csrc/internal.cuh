@@ -77,6 +77,10 @@ struct GrWindow {
     int64_t e_lo = 0, e_hi = 0;       // edges [e_lo,e_hi), e_lo rounded down to a multiple of 16
 };
 
+// hub filter of the enumeration kernels (hub_stride: sampled partial result; shard_*: one shard of a multi-GPU run)
+#define GR_HUB_SELECTED(v, i) (((v).hub_stride <= 1 || ((i) % (v).hub_stride) == 0) && \
+                               ((v).shard_count <= 1 || ((i) % (v).shard_count) == (v).shard_index))
+
 struct gramsci_graph {
     // parameters
     int64_t n = 0;
@@ -85,7 +89,7 @@ struct gramsci_graph {
     double box[3] = {0, 0, 0};
     double r_min = 0, r_max = 0;
     double q[GR_MAXBINS + 1];      // squared bin edges (A-3)
-    int weighted = 0, has_pix = 0, spatial = 0, algo = 0, hub_stride = 1;
+    int weighted = 0, has_pix = 0, spatial = 0, algo = 0, hub_stride = 1, shard_count = 1, shard_index = 0;
     cudaStream_t stream = nullptr;
     int sm_count = GR_SM_COUNT_FALLBACK;
     size_t smem_optin = 0;
@@ -146,6 +150,7 @@ struct GrView {
     int32_t s_lo, s_hi;     // schedule slots to walk (in-core: [0,n))
     const double *w;        // weights by label or nullptr
     int32_t hub_stride;     // > 1: only hubs with label % hub_stride == 0
+    int32_t shard_count, shard_index;   // shard_count > 1: only hubs with label % shard_count == shard_index
 };
 
 void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);

@@ -78,7 +78,7 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
         const int s = s_slot;
         if (s >= v.s_hi) break;
         const int32_t i = v.order[s];
-        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n >= 2) {
@@ -218,7 +218,7 @@ k_3pcf_merge(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
         const int s = s_slot;
         if (s >= v.s_hi) break;
         const int32_t i = v.order[s];
-        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n >= 2) {
@@ -425,7 +425,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             if (s_cur >= v.s_hi) break;
         }
         const int32_t i = v.order[s_cur++];
-        const bool mine = (i >= v.h_lo && i < v.h_hi) && (v.hub_stride <= 1 || (i % v.hub_stride) == 0);
+        const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n < 2) continue;

@@ -126,7 +126,7 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         const int s = s_slot;
         if (s >= v.s_hi) break;
         const int32_t i = v.order[s];
-        if (v.hub_stride > 1 && (i % v.hub_stride) != 0) continue;
+        if (!GR_HUB_SELECTED(v, i)) continue;
         const int64_t rb = v.ptr[i], re = v.ptr[i + 1];
         const int n = (int)(re - rb);
         if (n < 3) continue;                                   // a 4-clique needs three spokes
@@ -537,7 +537,7 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     }
 
     GrView v;
-    v.ptr = g->ptr.p; v.order = g->order.p; v.w = g->w.p; v.hub_stride = g->hub_stride;
+    v.ptr = g->ptr.p; v.order = g->order.p; v.w = g->w.p; v.hub_stride = g->hub_stride; v.shard_count = g->shard_count; v.shard_index = g->shard_index;
     v.idx_h = v.idx_c = g->idx.p; v.bin_h = v.bin_c = g->bin.p;
     v.pix_h = v.pix_c = g->has_pix ? g->pix.p : nullptr;
     v.e0_h = v.e0_c = 0;

@@ -31,6 +31,8 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     v.order = g->order.p;
     v.w = g->w.p;
     v.hub_stride = g->hub_stride;
+    v.shard_count = g->shard_count;
+    v.shard_index = g->shard_index;
     if (!g->ooc) {
         v.idx_h = v.idx_c = g->idx.p;
         v.bin_h = v.bin_c = g->bin.p;

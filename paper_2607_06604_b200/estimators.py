@@ -31,6 +31,12 @@ def zeta3_ratio(data_hist: np.ndarray, data_norm: float, rand_hist: np.ndarray, 
     return out
 
 
+def equilateral3(hist3: np.ndarray, nbins: int) -> np.ndarray:
+    """The equilateral 3pCF (P:135 names it as a separate kernel): the diagonal b1 = b2 = b3 of the dense histogram."""
+    h = np.asarray(hist3).reshape(nbins, nbins, nbins)
+    return np.array([h[b, b, b] for b in range(nbins)])
+
+
 def zeta4_connected(zeta4: np.ndarray, xi: np.ndarray) -> np.ndarray:
     """Eq. 5: zeta_conn = zeta - zeta_disc on the dense [nb^6] layout, zeta_disc from Eq. 4 through
     the library's host helper.  Applies to the even channel only."""

@@ -453,3 +453,31 @@ def test_full_size_config5_invariants_and_cap():
     c3c, _ = g2.pcf3()
     assert g2.timing(4) > 40e9                                          # the windows really were streamed
     assert np.array_equal(c3c, c3)
+
+
+def test_hub_shards_add_up_to_the_full_result():
+    """S:8(e): the hubs of one catalogue sharded over `shard_count` devices; the shard histograms sum to the full
+    result (exactly for counts) -- here the shards run one after the other on one GPU."""
+    cfg = small(51, n=4000, L=32.0, weighted=True, r_max=5.0, nb=5)
+    og = oracle.Graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    oc3, ow3 = og.pcf3()
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    for world in (2, 3):
+        c3 = np.zeros_like(oc3); w3 = np.zeros_like(ow3)
+        gec = np.zeros_like(ec); goc = np.zeros_like(oc); gew = np.zeros_like(ew); gow = np.zeros_like(ow)
+        for rank in range(world):
+            g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                       shard_count=world, shard_index=rank)
+            c, w = g.pcf3(weighted=True)
+            assert 0 < c.sum() < oc3.sum()
+            c3 += c; w3 += w
+            gp = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                        want_pixels=True, shard_count=world, shard_index=rank)
+            a, b, cc, d = gp.pcf4_parity(weighted=True)
+            gec += a; goc += b; gew += cc; gow += d
+        assert np.array_equal(c3, oc3) and np.array_equal(gec, ec) and np.array_equal(goc, oc)
+        assert_weighted_close(w3, ow3)
+        assert_weighted_close(gew, ew)
+        assert_weighted_close(gow, ow, scale=np.abs(ew))
+    with pytest.raises(gr.GramsciError):
+        gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], shard_count=2, shard_index=2)

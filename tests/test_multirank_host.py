@@ -34,6 +34,12 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
     fake_units = float(pts.shape[0] + rank)
     t = bench.max_over_ranks(fake_ms)
     u = bench.sum_over_ranks(fake_units)
+    # strong-scaling mode: partial histograms of the hub shards are summed with one all-reduce
+    part = np.arange(12, dtype=np.int64) * (rank + 1)
+    full = bench.allreduce_hist(part)
+    assert np.array_equal(full, np.arange(12, dtype=np.int64) * 3), full
+    wfull = bench.allreduce_hist(np.full(5, 0.25 * (rank + 1)))
+    assert np.allclose(wfull, 0.75)
     dist.barrier()
     np.save(os.path.join(out_dir, f"r{rank}.npy"), np.array([t, u, pts[0, 0], float(len(cats))]))
     dist.destroy_process_group()
