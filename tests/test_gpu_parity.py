@@ -481,3 +481,39 @@ def test_hub_shards_add_up_to_the_full_result():
         assert_weighted_close(gow, ow, scale=np.abs(ew))
     with pytest.raises(gr.GramsciError):
         gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], shard_count=2, shard_index=2)
+
+
+def test_many_bins_global_histogram_path():
+    """nb^3 bins beyond shared memory (40^3 x 4 B = 256 KB): the search kernel with a global histogram."""
+    cfg = small(61, n=2500, L=30.0, weighted=True, r_max=6.0, nb=40)
+    og, gg = build_both(cfg)
+    oc, ow = og.pcf3()
+    c, w = gg.pcf3(weighted=True)
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+    cfg1 = small(62, n=1500, L=30.0, r_min=2.0, r_max=6.0, nb=1)
+    og1, gg1 = build_both(cfg1)
+    assert np.array_equal(gg1.pcf3()[0], og1.pcf3()[0]) and np.array_equal(gg1.pcf4()[0], og1.pcf4()[0])
+
+
+def test_signed_weights():
+    """A-13: data-minus-random style weights of both signs; judged against sum |prod w| per bin."""
+    cfg = small(63, n=3000, L=30.0, r_max=5.0, nb=5)
+    rng = np.random.default_rng(64)
+    w = rng.uniform(0.5, 1.5, 3000) * rng.choice([-1.0, 1.0], 3000)
+    og = oracle.Graph(cfg["points"], w, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    oa = oracle.Graph(cfg["points"], np.abs(w), cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    for opts in (dict(), dict(algo=gr.ALGO_BSEARCH), dict(algo=gr.ALGO_MERGEPATH)):
+        gg = gr.gramsci_build_graph(cfg["points"], w, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], **opts)
+        c, ws = gg.pcf3(weighted=True)
+        assert np.array_equal(c, og.pcf3()[0])
+        assert_weighted_close(ws, og.pcf3()[1], scale=oa.pcf3()[1])
+        c2, w2 = gg.pcf2(weighted=True)
+        assert_weighted_close(w2, og.pcf2()[1], scale=oa.pcf2()[1])
+    gp = gr.gramsci_build_graph(cfg["points"], w, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], want_pixels=True)
+    ec, oc, ew, ow = gp.pcf4_parity(weighted=True)
+    rec, rew, roc, row = og.pcf4(parity=True)
+    sc = oa.pcf4()[1]
+    assert np.array_equal(ec, rec) and np.array_equal(oc, roc)
+    assert_weighted_close(ew, rew, scale=sc)
+    assert_weighted_close(ow, row, scale=sc)
