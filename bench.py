@@ -34,8 +34,8 @@ import catalogues as cat  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on cfg2, from the committed
 # ncu --set full capture (profiles/r1_c_table_3pcf_full.md)
-DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 577.233152e6 + 5.401344e6,
-                      "k_3pcf_table<counts>": 302.012672e6 + 4.176896e6}
+DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 576.641024e6 + 5.040896e6,
+                      "k_3pcf_table<counts>": 301.802240e6 + 3.864832e6}
 
 
 L2_READ_GBS = 12000.0      # L2 -> SM read bandwidth, 16-byte loads over a 32-64 MB working set (same micro-benchmark)
