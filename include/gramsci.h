@@ -115,6 +115,7 @@ int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edg
  * the caller labels j > i of its neighbours, ascending.  ptr int64 [N+1], idx int32 [E], bin uint8 [E],
  * pix uint8 [E] (only if built with want_pixels, else untouched).  HOST or DEVICE; any may be NULL.
  * With spatial relabelling the library converts (re-orients and re-sorts) on the device.
+ * Not available for graphs built under a device-memory cap (GRAMSCI_EINVAL).
  */
 int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t *idx, uint8_t *bin, uint8_t *pix);
 
@@ -125,7 +126,8 @@ int gramsci_2pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
 int gramsci_3pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
 
 /* 4pCF (S:8(a) A8, A10): every 4-clique once; [nb^6] at canonical 6-tuples.
- * Requires nbins <= 16. */
+ * Requires nbins <= 16, rows shorter than 65536 entries and a resident graph (no device-memory cap:
+ * GRAMSCI_EINVAL otherwise). */
 int gramsci_4pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
 
 /* Parity-decomposed 4pCF (Eq. 3; S:8(a) A9; A-8..A-11): even == gramsci_4pcf; odd adds

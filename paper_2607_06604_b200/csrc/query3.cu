@@ -31,13 +31,6 @@ struct Q3Params {
     int want_counts;
 };
 
-// ---- hub row staging ---------------------------------------------------------------------------------
-struct HubRow {
-    int32_t *idx;   // [row_cap]
-    uint8_t *bin;   // [row_cap]
-    double *w;      // [row_cap] (weighted only)
-};
-
 __device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31; }
 
 // lower_bound of key in sorted smem array a[lo,hi)
