@@ -9,6 +9,7 @@
 #include <map>
 #include <mutex>
 #include <thread>
+#include <tuple>
 #include <vector>
 #include <algorithm>
 #include <sys/mman.h>
@@ -58,6 +59,29 @@ bool gr_pools_supported()
         if (state < 0) { state = 0; cudaGetLastError(); }
     }
     return state == 1;
+}
+
+// ---- kernel attributes / occupancy, cached ---------------------------------------------------------------------
+int gr_kernel_occupancy(const void *fn, int threads, size_t smem)
+{
+    static std::mutex mu;
+    static std::map<std::tuple<int, const void *, size_t>, int> occ_cache;
+    static std::map<std::pair<int, const void *>, size_t> smem_set;
+    int dev = 0;
+    GR_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(mu);
+    auto &cur = smem_set[std::make_pair(dev, fn)];
+    if (smem > cur) {
+        GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        cur = smem;
+    }
+    const auto key = std::make_tuple(dev, fn, smem);
+    auto it = occ_cache.find(key);
+    if (it != occ_cache.end()) return it->second;
+    int occ = 0;
+    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem));
+    occ_cache[key] = occ;
+    return occ;
 }
 
 // ---- page-locked host memory -------------------------------------------------------------------------------

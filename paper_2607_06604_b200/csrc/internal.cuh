@@ -126,6 +126,10 @@ struct gramsci_graph {
     double t_build_ms = 0, t_query_ms = 0, t_enum_ms = 0, n_launches = 0, staged_bytes = 0;
 };
 
+// opt the kernel in to `smem` bytes of dynamic shared memory and return its resident CTAs per SM; both driver calls
+// are cached per (device, kernel, size) -- they cost a few hundred microseconds per query otherwise (api.cu)
+int gr_kernel_occupancy(const void *fn, int threads, size_t smem);
+
 // page-locked host memory for the out-of-core windows (api.cu): anonymous mapping, pages touched by all
 // host cores, then cudaHostRegister -- cudaHostAlloc pins at 2.6 GiB/s on this box, this path at ~25 GiB/s
 void *gr_pinned_alloc(size_t bytes);

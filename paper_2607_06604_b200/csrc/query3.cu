@@ -843,9 +843,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
         fn = W ? (const void *)k_3pcf_bsearch<true> : (const void *)k_3pcf_bsearch<false>;
     }
-    GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)r.smem));
-    int occ = 1;
-    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, Q3_THREADS, r.smem));
+    int occ = gr_kernel_occupancy(fn, Q3_THREADS, r.smem);
     occ = std::max(1, std::min(occ, 8));
     r.grid = g->sm_count * occ;
 

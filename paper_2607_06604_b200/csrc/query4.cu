@@ -496,9 +496,7 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
         GR_FAIL(GRAMSCI_ERANGE, "4pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
     const void *fn = small ? (use_lut ? (const void *)k_4pcf<true, true> : (const void *)k_4pcf<true, false>)
                            : (use_lut ? (const void *)k_4pcf<false, true> : (const void *)k_4pcf<false, false>);
-    GR_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int occ = 1;
-    GR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, Q4_THREADS, smem));
+    int occ = gr_kernel_occupancy(fn, Q4_THREADS, smem);
     occ = std::max(1, std::min(occ, 8));
     const int grid = g->sm_count * occ;
     const size_t stride = small ? 0 : ((mat_bytes + 255) & ~(size_t)255);
