@@ -10,8 +10,8 @@
 
 #define GR_MAXBINS 255
 #define GR_SM_COUNT_FALLBACK 148
-#define GR_S_MIN 3
-#define GR_S_MAX 12
+#define GR_S_MIN 4
+#define GR_S_MAX 11
 
 // ---- error plumbing --------------------------------------------------------------------------
 void gr_set_error(const char *fmt, ...);
