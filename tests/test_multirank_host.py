@@ -61,3 +61,19 @@ def test_single_process_reductions_are_identity():
     assert bench.max_over_ranks(3.5) == 3.5
     assert bench.sum_over_ranks(7.0) == 7.0
     assert bench.rank_seed_shift(0) == 0 and bench.rank_seed_shift(3) != bench.rank_seed_shift(2)
+
+
+def test_reference_arm_line_schema():
+    """bench.py --impl reference (the oracle on the host cores) prints one JSON line with the contract's keys."""
+    import json
+    import subprocess
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "cfg1",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, check=True, cwd=ROOT)
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                "scaling", "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in line, key
+    assert line["impl"] == "reference" and line["value"] > 0 and line["vs_baseline"] is None
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
+    assert line["config"]["workload"] == "cfg1"
