@@ -19,6 +19,9 @@
 
 namespace {
 
+#ifndef GR_LONG_U
+#define GR_LONG_U 8      // windows in flight per trip on long rows
+#endif
 constexpr int Q3_THREADS = 256;
 constexpr int Q3_WARPS = Q3_THREADS / 32;
 
@@ -721,8 +724,8 @@ void tile_3pcf(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
         if (r->p.weighted) k_3pcf_merge<true><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
         else k_3pcf_merge<false><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
     } else if (r->use_table) {
-        if (r->p.weighted) { if (r->long_rows) launch_table<true, 8>(r, v, st); else launch_table<true, 4>(r, v, st); }
-        else { if (r->long_rows) launch_table<false, 8>(r, v, st); else launch_table<false, 4>(r, v, st); }
+        if (r->p.weighted) { if (r->long_rows) launch_table<true, GR_LONG_U>(r, v, st); else launch_table<true, 4>(r, v, st); }
+        else { if (r->long_rows) launch_table<false, GR_LONG_U>(r, v, st); else launch_table<false, 4>(r, v, st); }
     } else if (r->p.weighted)
         k_3pcf_bsearch<true><<<r->grid, Q3_THREADS, r->smem, st>>>(v, r->p, r->counter, r->raw_cnt, r->raw_w);
     else
@@ -833,8 +836,8 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf: longest row (%d entries) does not fit in shared memory", g->max_row);
         fn = W ? (const void *)k_3pcf_merge<true> : (const void *)k_3pcf_merge<false>;
     } else if (r.use_table) {
-        fn = W ? (r.long_rows ? table_fn<true, 8>(r.G) : table_fn<true, 4>(r.G))
-               : (r.long_rows ? table_fn<false, 8>(r.G) : table_fn<false, 4>(r.G));
+        fn = W ? (r.long_rows ? table_fn<true, GR_LONG_U>(r.G) : table_fn<true, 4>(r.G))
+               : (r.long_rows ? table_fn<false, GR_LONG_U>(r.G) : table_fn<false, 4>(r.G));
     } else {
         r.p.smem_hist = ((size_t)nh * 4 <= 96 * 1024) ? 1 : 0;
         size_t per_entry = 4 + 1 + (W ? 8 : 0);
