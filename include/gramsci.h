@@ -30,6 +30,17 @@
  *
  * DETERMINISM.  Unweighted counts are exact integers, identical run to run and with or without a
  * device-memory cap.  Weighted fp64 sums may differ in the last bits with atomic order.
+ *
+ * THREADS.  The library keeps no process-global device state: build parameters and bin edges travel as
+ * kernel arguments, scratch is allocated per call.  Calls on DIFFERENT graphs may run concurrently from
+ * different host threads (each on its graph's stream); calls on the SAME graph must be serialised by the
+ * caller (a query records its timings and scratch in the graph, which is why the handle is not const
+ * in effect).  gramsci_last_error() is thread-local.
+ *
+ * DEVICE MEMORY.  The graph and all scratch come from the caller's allocator when gramsci_options.alloc /
+ * dealloc are set (the Python binding can pass PyTorch's caching allocator), else from a private
+ * stream-ordered memory pool of the device (never the device's default pool), which keeps freed blocks
+ * for the next call; gramsci_release_memory() returns them to the driver.
  */
 #ifndef GRAMSCI_H
 #define GRAMSCI_H
@@ -62,7 +73,10 @@ enum {
     GRAMSCI_ALGO_TABLE_G1 = 4,  /* slot table with a forced number of warps per hub: 1, 2, 4, 8          */
     GRAMSCI_ALGO_TABLE_G2 = 5,
     GRAMSCI_ALGO_TABLE_G4 = 6,
-    GRAMSCI_ALGO_TABLE_G8 = 7
+    GRAMSCI_ALGO_TABLE_G8 = 7,
+    GRAMSCI_ALGO_GATHER = 8,    /* dense cell-block rows + hub-tail gather (needs spatial labels); the default
+                                   when it applies                                                          */
+    GRAMSCI_ALGO_MAX = 8
 };
 
 typedef struct {       /* zero-initialised struct == defaults */
@@ -79,13 +93,20 @@ typedef struct {       /* zero-initialised struct == defaults */
                                       the paper's env-var override, P:159                                 */
     int hub_stride;                /* > 1: enumerate only tuples whose smallest-label vertex i has i % hub_stride
                                       == 0 (a sampled partial result, for checking full-size runs against a
-                                      reference that is too slow to run in full); needs caller labels
-                                      (relabel = 2 or want_pixels), else GRAMSCI_EINVAL                    */
+                                      reference that is too slow to run in full).  The label is the INTERNAL
+                                      one: the caller's with relabel = 2 / want_pixels, else the cell-order label
+                                      that gramsci_export_labels returns                                   */
     int shard_count, shard_index;  /* shard_count > 1: this graph's queries enumerate only the tuples whose hub (the
                                       vertex with the smallest internal label) has label % shard_count ==
                                       shard_index.  The shards partition the tuples: the histograms of shards
                                       0..shard_count-1 add up to the full result, exactly for counts -- one GPU
                                       per shard and one all-reduce of the histogram (S:8(e)); 2pCF is not sharded */
+    int reserved;                  /* must be 0 */
+    /* Device allocator hooks (S:8(b)): both or neither.  alloc returns a DEVICE pointer valid on `stream`
+       (256-byte aligned) or NULL; dealloc releases it.  NULL = the library's private memory pool.       */
+    void *(*alloc)(size_t bytes, void *stream, void *user);
+    void (*dealloc)(void *ptr, void *stream, void *user);
+    void *user;
 } gramsci_options;
 
 /*
@@ -118,6 +139,11 @@ int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edg
  * Not available for graphs built under a device-memory cap (GRAMSCI_EINVAL).
  */
 int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t *idx, uint8_t *bin, uint8_t *pix);
+
+/* Internal label -> caller label (HOST or DEVICE int32 [N]): caller_of[l] is the index, in the caller's points
+ * array, of the point with internal label l.  Identity when the graph keeps caller labels.  With it a caller can
+ * reproduce the internal order (hub_stride, shard_* and the hub of a tuple are defined on internal labels). */
+int gramsci_export_labels(const gramsci_graph *g, int32_t *caller_of);
 
 /* 2pCF sweep (S:8(a) A6): counts[b] = #edges in bin b, wsum[b] = sum w_i w_j.  [nb] each. */
 int gramsci_2pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
@@ -161,6 +187,10 @@ int gramsci_last_timing(const gramsci_graph *g, int what, double *value);
 int gramsci_work_counters(const gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
 
 void gramsci_free_graph(gramsci_graph *g);
+
+/* Return the freed blocks of the library's private memory pool on the current device to the driver
+ * (synchronises the device).  Graphs larger than 4 GiB trim the pool to 2 GiB when they are freed. */
+int gramsci_release_memory(void);
 
 const char *gramsci_last_error(void); /* thread-local, never NULL */
 

@@ -25,10 +25,12 @@ ABI_SYMBOLS = [
     "gramsci_build_graph", "gramsci_graph_info", "gramsci_export_csr", "gramsci_2pcf", "gramsci_3pcf",
     "gramsci_4pcf", "gramsci_4pcf_parity", "gramsci_num_configs", "gramsci_compact", "gramsci_zeta_disc",
     "gramsci_last_timing", "gramsci_work_counters", "gramsci_free_graph", "gramsci_last_error",
+    "gramsci_export_labels", "gramsci_release_memory",
 ]
 
 ALGO_DEFAULT, ALGO_MERGEPATH, ALGO_BSEARCH, ALGO_BITMAP = 0, 1, 2, 3
 ALGO_TABLE_G1, ALGO_TABLE_G2, ALGO_TABLE_G4, ALGO_TABLE_G8 = 4, 5, 6, 7
+ALGO_GATHER = 8
 
 STATUS = {0: "GRAMSCI_OK", 1: "GRAMSCI_EINVAL", 2: "GRAMSCI_ERANGE", 3: "GRAMSCI_ENOMEM", 4: "GRAMSCI_ECUDA",
           5: "GRAMSCI_EOVERFLOW"}
@@ -40,11 +42,33 @@ class GramsciError(RuntimeError):
         self.code = code
 
 
+_ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p)
+_DEALLOC_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p)
+
+
 class _Options(ctypes.Structure):
     _fields_ = [("stream", ctypes.c_void_p), ("device_mem_cap_bytes", ctypes.c_uint64),
                 ("want_pixels", ctypes.c_int), ("relabel", ctypes.c_int), ("algo", ctypes.c_int),
                 ("n_windows", ctypes.c_int), ("hub_stride", ctypes.c_int),
-                ("shard_count", ctypes.c_int), ("shard_index", ctypes.c_int)]
+                ("shard_count", ctypes.c_int), ("shard_index", ctypes.c_int), ("reserved", ctypes.c_int),
+                ("alloc", _ALLOC_FN), ("dealloc", _DEALLOC_FN), ("user", ctypes.c_void_p)]
+
+
+def _torch_alloc(size, stream, user):
+    """``gramsci_options.alloc`` hook: PyTorch's caching allocator (device memory belongs to torch)."""
+    import torch
+    try:
+        return torch.cuda.caching_allocator_alloc(int(size), stream=int(stream or 0))
+    except Exception:        # out of memory: the library reports GRAMSCI_ENOMEM
+        return None
+
+
+def _torch_dealloc(ptr, stream, user):
+    import torch
+    torch.cuda.caching_allocator_delete(int(ptr))
+
+
+_TORCH_HOOKS = (_ALLOC_FN(_torch_alloc), _DEALLOC_FN(_torch_dealloc))     # kept alive for the life of the process
 
 
 _lib = None
@@ -86,6 +110,10 @@ def load_library():
     L.gramsci_free_graph.argtypes = [vp]
     L.gramsci_last_error.restype = ctypes.c_char_p
     L.gramsci_last_error.argtypes = []
+    L.gramsci_export_labels.restype = ctypes.c_int
+    L.gramsci_export_labels.argtypes = [vp, vp]
+    L.gramsci_release_memory.restype = ctypes.c_int
+    L.gramsci_release_memory.argtypes = []
     _lib = L
     return L
 
@@ -161,6 +189,12 @@ class Graph:
         _check(load_library().gramsci_export_csr(self._h, _ptr(ptr), _ptr(idx), _ptr(b), _ptr(p)))
         return (ptr, idx[:e], b[:e], p[:e]) if want_pix else (ptr, idx[:e], b[:e])
 
+    def export_labels(self) -> np.ndarray:
+        """``gramsci_export_labels``: caller index of every internal label (int32 [N], host)."""
+        out = np.zeros(max(self.info()["n_points"], 1), dtype=np.int32)
+        _check(load_library().gramsci_export_labels(self._h, _ptr(out)))
+        return out[:self.info()["n_points"]]
+
     # -- outputs ------------------------------------------------------------------------------------
     def _out(self, n: int, dtype: str, host: bool):
         if host or not self._device_outputs:
@@ -211,7 +245,7 @@ class Graph:
 def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = None, r_min: float = 0.0,
                         r_max: float = 1.0, nbins: int = 1, *, want_pixels: bool = False, relabel: int = 0,
                         algo: int = 0, device_mem_cap_bytes: int = 0, n_windows: int = 0, hub_stride: int = 0,
-                        shard_count: int = 0, shard_index: int = 0) -> Graph:
+                        shard_count: int = 0, shard_index: int = 0, torch_allocator: bool = False) -> Graph:
     """``gramsci_build_graph`` (include/gramsci.h).  ``points`` [N,3] / ``weights`` [N] fp64: torch CUDA
     tensors (used in place), torch CPU tensors or NumPy arrays (the library stages host buffers itself)."""
     L = load_library()
@@ -238,6 +272,8 @@ def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = N
     opt.hub_stride = int(hub_stride)
     opt.shard_count = int(shard_count)
     opt.shard_index = int(shard_index)
+    if torch_allocator:          # S:8(b): the graph and all scratch come from torch's caching allocator
+        opt.alloc, opt.dealloc = _TORCH_HOOKS
     cbox = None
     if box is not None:
         cbox = (ctypes.c_double * 3)(*[float(v) for v in box])
@@ -248,6 +284,10 @@ def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = N
     _check(code)
     device = _is_torch(points) and points.is_cuda
     return Graph(h.value, int(nbins), device)
+
+
+def gramsci_release_memory() -> None:
+    _check(load_library().gramsci_release_memory())
 
 
 def gramsci_num_configs(npoint: int, nbins: int) -> int:

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -35,30 +36,92 @@ extern "C" const char *gramsci_last_error(void) { return t_err; }
     catch (...) { gr_set_error("unexpected internal error"); return GRAMSCI_ECUDA; }                  \
     return GRAMSCI_OK;
 
-// ---- allocation stream / pools ---------------------------------------------------------------------------
-cudaStream_t &gr_alloc_stream()
+// ---- allocation context / private memory pool ----------------------------------------------------------------
+GrAllocCtx &gr_alloc_ctx()
 {
-    static thread_local cudaStream_t st = nullptr;
-    return st;
+    static thread_local GrAllocCtx ctx;
+    return ctx;
 }
 
-bool gr_pools_supported()
+// one private pool per device (nullptr = pools unsupported on that device: plain cudaMalloc)
+static std::mutex g_pool_mu;
+static std::map<int, cudaMemPool_t> g_pools;
+
+static cudaMemPool_t gr_pool(int dev)
 {
-    static int state = -1;                 // -1 unknown, 0 no, 1 yes
-    if (state < 0) {
-        int dev = 0, ok = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&ok, cudaDevAttrMemoryPoolsSupported, dev) == cudaSuccess && ok) {
-            cudaMemPool_t pool;
-            if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                uint64_t thr = UINT64_MAX;
-                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-                state = 1;
-            }
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    auto it = g_pools.find(dev);
+    if (it != g_pools.end()) return it->second;
+    cudaMemPool_t pool = nullptr;
+    int ok = 0;
+    if (cudaDeviceGetAttribute(&ok, cudaDevAttrMemoryPoolsSupported, dev) == cudaSuccess && ok) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if (cudaMemPoolCreate(&pool, &props) == cudaSuccess) {
+            uint64_t thr = UINT64_MAX;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        } else {
+            pool = nullptr;
         }
-        if (state < 0) { state = 0; cudaGetLastError(); }
     }
-    return state == 1;
+    cudaGetLastError();
+    g_pools[dev] = pool;
+    return pool;
+}
+
+void *gr_dev_alloc(size_t bytes, const GrAllocCtx &ctx, int *kind)
+{
+    void *p = nullptr;
+    if (ctx.alloc) {
+        p = ctx.alloc(bytes, (void *)ctx.stream, ctx.user);
+        if (!p) GR_FAIL(GRAMSCI_ENOMEM, "the caller's allocator returned NULL for %zu bytes", bytes);
+        *kind = 2;
+        return p;
+    }
+    int dev = 0;
+    GR_CUDA(cudaGetDevice(&dev));
+    cudaMemPool_t pool = gr_pool(dev);
+    if (pool) {
+        GR_CUDA(cudaMallocFromPoolAsync(&p, bytes, pool, ctx.stream));
+        *kind = 1;
+    } else {
+        GR_CUDA(cudaMalloc(&p, bytes));
+        *kind = 0;
+    }
+    return p;
+}
+
+void gr_dev_free(void *p, const GrAllocCtx &ctx, int kind)
+{
+    if (!p) return;
+    if (kind == 2) { if (ctx.dealloc) ctx.dealloc(p, (void *)ctx.stream, ctx.user); }
+    else if (kind == 1) cudaFreeAsync(p, ctx.stream);
+    else cudaFree(p);
+}
+
+extern "C" int gramsci_release_memory(void)
+{
+    GR_API_BEGIN
+    int dev = 0;
+    GR_CUDA(cudaGetDevice(&dev));
+    cudaMemPool_t pool = gr_pool(dev);
+    if (pool) {
+        GR_CUDA(cudaDeviceSynchronize());
+        GR_CUDA(cudaMemPoolTrimTo(pool, 0));
+    }
+    GR_API_END
+}
+
+unsigned long long gr_flush_budget(unsigned long long dflt)
+{
+    const char *e = getenv("GRAMSCI_FLUSH_BUDGET");
+    if (!e || !*e) return dflt;
+    const unsigned long long v = strtoull(e, nullptr, 10);
+    return (v >= 1 && v < dflt) ? v : dflt;
 }
 
 // ---- kernel attributes / occupancy, cached ---------------------------------------------------------------------
@@ -195,7 +258,7 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     gramsci_options o;
     memset(&o, 0, sizeof o);
     if (opt) o = *opt;
-    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > 7 || o.n_windows < 0 || o.hub_stride < 0 ||
+    if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > GRAMSCI_ALGO_MAX || o.n_windows < 0 || o.hub_stride < 0 ||
         o.shard_count < 0 || o.shard_index < 0 || (o.shard_count > 1 && o.shard_index >= o.shard_count))
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: bad options");
     require_device();
@@ -230,9 +293,9 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->hub_stride = o.hub_stride > 1 ? o.hub_stride : 1;
     g->shard_count = o.shard_count > 1 ? o.shard_count : 1;
     g->shard_index = o.shard_count > 1 ? o.shard_index : 0;
-    if (g->hub_stride > 1 && g->spatial) {
+    if (g->has_pix && g->spatial) {
         delete g; g = nullptr;
-        GR_FAIL(GRAMSCI_EINVAL, "build_graph: hub_stride needs caller labels (relabel = 2 or want_pixels)");
+        GR_FAIL(GRAMSCI_EINVAL, "build_graph: want_pixels needs caller labels (A-10): relabel = 1 cannot be combined with it");
     }
     g->stream = (cudaStream_t)o.stream;
     g->cap_bytes = o.device_mem_cap_bytes;
@@ -253,7 +316,12 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
         g->smem_optin = it->second.second;
     }
 
-    gr_alloc_stream() = g->stream;
+    if ((o.alloc != nullptr) != (o.dealloc != nullptr)) {
+        delete g; g = nullptr;
+        GR_FAIL(GRAMSCI_EINVAL, "build_graph: alloc and dealloc must be given together");
+    }
+    g->actx.stream = g->stream; g->actx.alloc = o.alloc; g->actx.dealloc = o.dealloc; g->actx.user = o.user;
+    gr_alloc_ctx() = g->actx;
     DevBuf<double> hp, hw;
     const double *d_pts = stage_in(points, (size_t)N * 3, hp, g->stream);
     const double *d_w = stage_in(weights, (size_t)N, hw, g->stream);
@@ -275,7 +343,18 @@ extern "C" void gramsci_free_graph(gramsci_graph *g)
     gr_pinned_free(g->h_idx, g->h_idx_bytes);
     gr_pinned_free(g->h_bin, g->h_bin_bytes);
     gr_pinned_free(g->h_pix, g->h_pix_bytes);
+    const bool big = (uint64_t)g->n_edges * 5 > ((uint64_t)4 << 30) && !g->actx.alloc;
+    cudaStream_t st = g->stream;
     delete g;
+    if (big) {      // do not sit on tens of GB of freed blocks: other users of the device (PyTorch) cannot see them
+        int dev = 0;
+        cudaStreamSynchronize(st);
+        if (cudaGetDevice(&dev) == cudaSuccess) {
+            cudaMemPool_t pool = gr_pool(dev);
+            if (pool) cudaMemPoolTrimTo(pool, (size_t)2 << 30);
+        }
+        cudaGetLastError();
+    }
 }
 
 extern "C" int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edges, int32_t *max_row,
@@ -295,7 +374,7 @@ extern "C" int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t 
 {
     GR_API_BEGIN
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "export_csr: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     OutStage<int64_t> op; OutStage<int32_t> oi; OutStage<uint8_t> ob, ox;
     op.init(ptr, (size_t)g->n + 1);
     oi.init(idx, (size_t)g->n_edges);
@@ -306,13 +385,38 @@ extern "C" int gramsci_export_csr(const gramsci_graph *g, int64_t *ptr, int32_t 
     GR_API_END
 }
 
+__global__ void k_iota(int32_t *out, int64_t n)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = (int32_t)i;
+}
+
+extern "C" int gramsci_export_labels(const gramsci_graph *g, int32_t *caller_of)
+{
+    GR_API_BEGIN
+    if (!g) GR_FAIL(GRAMSCI_EINVAL, "export_labels: NULL graph");
+    gr_alloc_ctx() = g->actx;
+    OutStage<int32_t> o;
+    o.init(caller_of, (size_t)g->n);
+    if (caller_of && g->n > 0) {
+        if (g->spatial)
+            GR_CUDA(cudaMemcpyAsync(o.dev, g->caller_of.p, sizeof(int32_t) * g->n, cudaMemcpyDeviceToDevice, g->stream));
+        else
+            k_iota<<<(unsigned)((g->n + 255) / 256), 256, 0, g->stream>>>(o.dev, g->n);
+        GR_CUDA(cudaGetLastError());
+        GR_CUDA(cudaStreamSynchronize(g->stream));
+    }
+    o.finish(g->stream);
+    GR_API_END
+}
+
 // ---- queries -----------------------------------------------------------------------------------------------
 extern "C" int gramsci_2pcf(const gramsci_graph *cg, uint64_t *counts, double *wsum)
 {
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "2pcf: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     OutStage<uint64_t> oc; OutStage<double> ow;
     oc.init(counts, (size_t)g->nb);
     ow.init(wsum, (size_t)g->nb);
@@ -326,7 +430,7 @@ extern "C" int gramsci_3pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "3pcf: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     const size_t nh = (size_t)ipow(g->nb, 3);
     OutStage<uint64_t> oc; OutStage<double> ow;
     oc.init(counts, nh);
@@ -341,7 +445,7 @@ extern "C" int gramsci_4pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "4pcf: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     if (g->nb > 16) GR_FAIL(GRAMSCI_EINVAL, "4pcf: nbins must be <= 16");
     const size_t nh = (size_t)ipow(g->nb, 6);
     OutStage<uint64_t> oc; OutStage<double> ow;
@@ -358,7 +462,7 @@ extern "C" int gramsci_4pcf_parity(const gramsci_graph *cg, uint64_t *even_count
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     if (g->nb > 16) GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: nbins must be <= 16");
     if (!g->has_pix || g->spatial)
         GR_FAIL(GRAMSCI_EINVAL, "4pcf_parity: graph must be built with want_pixels=1 in caller-label order (A-10)");
@@ -393,7 +497,7 @@ extern "C" int gramsci_work_counters(const gramsci_graph *cg, uint64_t *spoke_el
     GR_API_BEGIN
     gramsci_graph *g = const_cast<gramsci_graph *>(cg);
     if (!g) GR_FAIL(GRAMSCI_EINVAL, "work_counters: NULL graph");
-    gr_alloc_stream() = g->stream;
+    gr_alloc_ctx() = g->actx;
     gr_work_counters(g, spoke_elems, tail_elems);
     GR_API_END
 }

@@ -15,6 +15,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 
 namespace {
 
@@ -29,23 +30,26 @@ struct BuildParams {
     int want_pix;
 };
 
-__constant__ double c_q[GR_MAXBINS + 1];   // squared bin edges
-__constant__ BuildParams c_bp;
+struct BinEdges { double q[GR_MAXBINS + 1]; };   // squared bin edges (A-3)
+
+// Both structs travel as __grid_constant__ kernel parameters (the parameter bank is constant memory): nothing
+// about a build lives in process-global device state, so builds on different streams or host threads do not
+// touch each other (include/gramsci.h, THREADS).
 
 // ---- A1: cell ids ------------------------------------------------------------------------------
-__device__ __forceinline__ int cell_coord(double x, int c)
+__device__ __forceinline__ int cell_coord(const BuildParams &c_bp, double x, int c)
 {
     int k = (int)floor((x - c_bp.lo[c]) * c_bp.inv_cw[c]);
     k = max(0, min(k, c_bp.nc[c] - 1));
     return k;
 }
 
-__global__ void k_cell_id(const double *__restrict__ pts, int32_t *__restrict__ cell_of,
-                          int32_t *__restrict__ cell_cnt)
+__global__ void k_cell_id(const __grid_constant__ BuildParams c_bp, const double *__restrict__ pts,
+                          int32_t *__restrict__ cell_of, int32_t *__restrict__ cell_cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c_bp.n) return;
-    int cx = cell_coord(pts[3 * i + 0], 0), cy = cell_coord(pts[3 * i + 1], 1), cz = cell_coord(pts[3 * i + 2], 2);
+    int cx = cell_coord(c_bp, pts[3 * i + 0], 0), cy = cell_coord(c_bp, pts[3 * i + 1], 1), cz = cell_coord(c_bp, pts[3 * i + 2], 2);
     int id = (cz * c_bp.nc[1] + cy) * c_bp.nc[0] + cx;
     cell_of[i] = id;
     atomicAdd(&cell_cnt[id], 1);
@@ -63,11 +67,13 @@ __global__ void k_scatter_cells(const int32_t *__restrict__ cell_of, int32_t *__
 // gather coordinates (SoA) and labels into slot order
 __global__ void k_gather_slots(const double *__restrict__ pts, const int32_t *__restrict__ slot_pt,
                                double *__restrict__ sx, double *__restrict__ sy, double *__restrict__ sz,
-                               int32_t *__restrict__ lab, int32_t *__restrict__ caller_of, int64_t n, int spatial)
+                               int32_t *__restrict__ lab, int32_t *__restrict__ caller_of,
+                               const int32_t *__restrict__ cell_of, int32_t *__restrict__ cell_of_slot, int64_t n, int spatial)
 {
     int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     int32_t i = slot_pt[s];
+    if (cell_of_slot) cell_of_slot[s] = cell_of[i];
     sx[s] = pts[3 * (int64_t)i + 0];
     sy[s] = pts[3 * (int64_t)i + 1];
     sz[s] = pts[3 * (int64_t)i + 2];
@@ -111,8 +117,8 @@ __global__ void k_minmax(const double *__restrict__ pts, int64_t n, double *__re
 // ---- A3: exclusive prefix sum, int32 counts -> int64 offsets (three-phase scan) -----------------------
 constexpr int SCAN_BLOCK = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_BLOCK * SCAN_ITEMS;
 
-template <typename OutT>
-__global__ void k_scan_tile_sums(const int32_t *__restrict__ in, int64_t n, int64_t *__restrict__ tile_sum)
+template <typename InT>
+__global__ void k_scan_tile_sums(const InT *__restrict__ in, int64_t n, int64_t *__restrict__ tile_sum)
 {
     __shared__ int64_t s[SCAN_BLOCK];
     int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
@@ -155,14 +161,14 @@ __global__ void k_scan_tile_offsets(int64_t *__restrict__ tile_sum, int64_t n_ti
     }
 }
 
-template <typename OutT>
-__global__ void k_scan_apply(const int32_t *__restrict__ in, int64_t n, const int64_t *__restrict__ tile_off,
+template <typename InT, typename OutT>
+__global__ void k_scan_apply(const InT *__restrict__ in, int64_t n, const int64_t *__restrict__ tile_off,
                              OutT *__restrict__ out)
 {
     // each thread owns SCAN_ITEMS consecutive items
     __shared__ int64_t s[SCAN_BLOCK];
     int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
-    int32_t v[SCAN_ITEMS];
+    InT v[SCAN_ITEMS];
     int64_t acc = 0;
     for (int k = 0; k < SCAN_ITEMS; ++k) {
         v[k] = (base + k < n) ? in[base + k] : 0;
@@ -184,8 +190,8 @@ __global__ void k_scan_apply(const int32_t *__restrict__ in, int64_t n, const in
     if (base <= n - 1 && n - 1 < base + SCAN_ITEMS) out[n] = (OutT)run;   // total
 }
 
-template <typename OutT>
-void exclusive_scan(const int32_t *d_in, int64_t n, OutT *d_out, cudaStream_t st)
+template <typename OutT, typename InT = int32_t>
+void exclusive_scan(const InT *d_in, int64_t n, OutT *d_out, cudaStream_t st)
 {
     if (n == 0) {
         GR_CUDA(cudaMemsetAsync(d_out, 0, sizeof(OutT), st));
@@ -194,9 +200,9 @@ void exclusive_scan(const int32_t *d_in, int64_t n, OutT *d_out, cudaStream_t st
     int64_t tiles = (n + SCAN_TILE - 1) / SCAN_TILE;
     DevBuf<int64_t> ts;
     ts.alloc((size_t)tiles);
-    k_scan_tile_sums<OutT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p);
+    k_scan_tile_sums<InT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p);
     k_scan_tile_offsets<<<1, 1024, 0, st>>>(ts.p, tiles);
-    k_scan_apply<OutT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p, d_out);
+    k_scan_apply<InT, OutT><<<(unsigned)tiles, SCAN_BLOCK, 0, st>>>(d_in, n, ts.p, d_out);
     GR_CUDA(cudaGetLastError());
     GR_CUDA(cudaStreamSynchronize(st));   // ts freed on return
 }
@@ -288,12 +294,12 @@ k_segsort(const OffT *__restrict__ seg, int64_t seg_lo, int64_t seg_hi, int64_t 
 }
 
 // ---- A2 / A4: neighbour count and fill ------------------------------------------------------------------
-__device__ __forceinline__ int bin_of(double d2)
+__device__ __forceinline__ int bin_of(const BuildParams &c_bp, const BinEdges &eq, double d2)
 {   // b = #{k in [1,nb): q_k <= d2} (A-3); q is non-decreasing so this is an upper bound search
     int lo = 1, hi = c_bp.nb;            // answer = (first k in [1,nb) with q_k > d2) - 1
     while (lo < hi) {
         int mid = (lo + hi) >> 1;
-        if (c_q[mid] <= d2) lo = mid + 1; else hi = mid;
+        if (eq.q[mid] <= d2) lo = mid + 1; else hi = mid;
     }
     return lo - 1;
 }
@@ -320,7 +326,8 @@ __device__ __forceinline__ int pixel_of(double dx, double dy, double dz, double 
 // ascending id so that in spatial mode (label == slot) the row is emitted already sorted (Eq. 1).
 template <bool FILL>
 __global__ void __launch_bounds__(256)
-k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const double *__restrict__ sz,
+k_neighbours(const __grid_constant__ BuildParams c_bp, const __grid_constant__ BinEdges eq,
+             const double *__restrict__ sx, const double *__restrict__ sy, const double *__restrict__ sz,
              const int32_t *__restrict__ lab, const int32_t *__restrict__ cell_start,
              int64_t slot_lo, int64_t slot_hi, int32_t row_lo, int32_t row_hi,
              int32_t *__restrict__ deg, const int64_t *__restrict__ ptr, int64_t e0,
@@ -332,7 +339,7 @@ k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const
     const int32_t li = lab[s];
     if (li < row_lo || li >= row_hi) return;
     const double xi = sx[s], yi = sy[s], zi = sz[s];
-    const int cx = cell_coord(xi, 0), cy = cell_coord(yi, 1), cz = cell_coord(zi, 2);
+    const int cx = cell_coord(c_bp, xi, 0), cy = cell_coord(c_bp, yi, 1), cz = cell_coord(c_bp, zi, 2);
     const int own = (cz * c_bp.nc[1] + cy) * c_bp.nc[0] + cx;
 
     // stencil cell of this lane
@@ -389,7 +396,7 @@ k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const
     const bool per = c_bp.periodic != 0;
     const double hx = per ? c_bp.half[0] : INFINITY, hy = per ? c_bp.half[1] : INFINITY, hz = per ? c_bp.half[2] : INFINITY;
     const double bx = c_bp.box[0], by = c_bp.box[1], bz = c_bp.box[2];
-    const double q_lo = c_q[0], q_hi = c_q[c_bp.nb];
+    const double q_lo = eq.q[0], q_hi = eq.q[c_bp.nb];
     // separation component a -> b, minimum image when periodic (A-4); half = +inf switches the wrap off
     auto sep = [](double a, double b, double half, double box) -> double {
         double d = __dsub_rn(b, a);
@@ -425,7 +432,7 @@ k_neighbours(const double *__restrict__ sx, const double *__restrict__ sy, const
             const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
             edge = (d2 >= q_lo) && (d2 < q_hi);                // r_min <= r < r_max (A-2)
             if (FILL && edge) {
-                bb = bin_of(d2);
+                bb = bin_of(c_bp, eq, d2);
                 if (c_bp.want_pix) pp = pixel_of(dx, dy, dz, d2);
             }
         }
@@ -573,6 +580,25 @@ __global__ void k_need_mask(const int32_t *__restrict__ idx, int64_t lo, int64_t
 
 inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64_t>(1, (n + per - 1) / per); }
 
+// min and max of |w| (fp64 atomics on two words; doubles >= 0 order like their bit patterns)
+__global__ void k_abs_minmax(const double *__restrict__ w, int64_t n, double *__restrict__ out)
+{
+    double mn = INFINITY, mx = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const double a = fabs(w[i]);
+        mn = fmin(mn, a);
+        mx = fmax(mx, a);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin((unsigned long long *)&out[0], (unsigned long long)__double_as_longlong(mn));
+        atomicMax((unsigned long long *)&out[1], (unsigned long long)__double_as_longlong(mx));
+    }
+}
+
 template <typename OffT>
 __global__ void k_seg_max(const OffT *__restrict__ seg, int64_t n, int32_t *__restrict__ out)
 {
@@ -619,6 +645,15 @@ void gr_exclusive_scan_i32(const int32_t *d_in, int64_t n, int32_t *d_out, cudaS
 {
     exclusive_scan<int32_t>(d_in, n, d_out, st);
 }
+
+template <typename InT, typename OutT>
+void gr_exclusive_scan(const InT *d_in, int64_t n, OutT *d_out, cudaStream_t st)
+{
+    exclusive_scan<OutT, InT>(d_in, n, d_out, st);
+}
+template void gr_exclusive_scan<int32_t, int32_t>(const int32_t *, int64_t, int32_t *, cudaStream_t);
+template void gr_exclusive_scan<int32_t, int64_t>(const int32_t *, int64_t, int64_t *, cudaStream_t);
+template void gr_exclusive_scan<int64_t, int64_t>(const int64_t *, int64_t, int64_t *, cudaStream_t);
 
 // ---------------------------------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced)
@@ -677,13 +712,13 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         // guard: rounding in (x-lo)*inv_cw must not push two points closer than r_max two cells apart
         bp.inv_cw[c] *= (1.0 - 1e-12);
     }
-    GR_CUDA(cudaMemcpyToSymbolAsync(c_bp, &bp, sizeof(bp), 0, cudaMemcpyHostToDevice, st));
-    GR_CUDA(cudaMemcpyToSymbolAsync(c_q, g->q, sizeof(double) * (g->nb + 1), 0, cudaMemcpyHostToDevice, st));
+    BinEdges eq;
+    for (int k = 0; k <= GR_MAXBINS; ++k) eq.q[k] = (k <= g->nb) ? g->q[k] : INFINITY;
 
     g->ptr.alloc((size_t)n + 1);
     g->w.alloc((size_t)n);
     g->order.alloc((size_t)n);
-    if (g->spatial) g->caller_of.alloc((size_t)n);
+    if (g->spatial) { g->caller_of.alloc((size_t)n); g->cell_of.alloc((size_t)n); }
     if (n == 0) {
         GR_CUDA(cudaMemsetAsync(g->ptr.p, 0, sizeof(int64_t), st));
         g->idx.alloc(0); g->bin.alloc(0);
@@ -698,14 +733,16 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     }
 
     // --- counting sort of the points by cell, ascending caller index inside a cell (A1) ---
-    DevBuf<int32_t> cell_of, cell_cnt, cell_start, cell_fill, slot_pt;
+    DevBuf<int32_t> cell_of, cell_cnt, cell_fill, slot_pt;
+    DevBuf<int32_t> &cell_start = g->cell_start;      // kept: the dense cell-block rows are laid out by cell (dense.cu)
+    g->ncell = ncell;
     cell_of.alloc((size_t)n);
     cell_cnt.alloc((size_t)ncell);
     cell_start.alloc((size_t)ncell + 1);
     cell_fill.alloc((size_t)ncell + 1);
     slot_pt.alloc((size_t)n);
     GR_CUDA(cudaMemsetAsync(cell_cnt.p, 0, sizeof(int32_t) * ncell, st));
-    k_cell_id<<<blocks_for(n, 256), 256, 0, st>>>(d_points, cell_of.p, cell_cnt.p);
+    k_cell_id<<<blocks_for(n, 256), 256, 0, st>>>(bp, d_points, cell_of.p, cell_cnt.p);
     exclusive_scan<int32_t>(cell_cnt.p, ncell, cell_start.p, st);
     GR_CUDA(cudaMemcpyAsync(cell_fill.p, cell_start.p, sizeof(int32_t) * (ncell + 1), cudaMemcpyDeviceToDevice, st));
     k_scatter_cells<<<blocks_for(n, 256), 256, 0, st>>>(cell_of.p, cell_fill.p, slot_pt.p, n);
@@ -716,7 +753,8 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     DevBuf<int32_t> lab;
     sx.alloc((size_t)n); sy.alloc((size_t)n); sz.alloc((size_t)n); lab.alloc((size_t)n);
     k_gather_slots<<<blocks_for(n, 256), 256, 0, st>>>(d_points, slot_pt.p, sx.p, sy.p, sz.p, lab.p,
-                                                       g->spatial ? g->caller_of.p : nullptr, n, g->spatial);
+                                                       g->spatial ? g->caller_of.p : nullptr, cell_of.p,
+                                                       g->spatial ? g->cell_of.p : nullptr, n, g->spatial);
     k_gather_weights<<<blocks_for(n, 256), 256, 0, st>>>(d_weights, slot_pt.p, g->w.p, n, g->spatial);
     GR_CUDA(cudaMemcpyAsync(g->order.p, lab.p, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, st));
     launches += 2;
@@ -725,7 +763,7 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     DevBuf<int32_t> deg;
     deg.alloc((size_t)n);
     const unsigned nblk = blocks_for(n * 32, 256);
-    k_neighbours<false><<<nblk, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, deg.p,
+    k_neighbours<false><<<nblk, 256, 0, st>>>(bp, eq, sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, deg.p,
                                               nullptr, 0, nullptr, nullptr, nullptr);
     exclusive_scan<int64_t>(deg.p, n, g->ptr.p, st);
     launches += 4;
@@ -790,16 +828,14 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         g->idx.alloc((size_t)E);
         g->bin.alloc((size_t)E);
         if (g->has_pix) g->pix.alloc((size_t)E);
-        k_neighbours<true><<<nblk, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, nullptr,
+        k_neighbours<true><<<nblk, 256, 0, st>>>(bp, eq, sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, nullptr,
                                                  g->ptr.p, 0, g->idx.p, g->bin.p, g->has_pix ? g->pix.p : nullptr);
         launches += 1;
         if (!g->spatial) {
             segsort<int64_t>(g->ptr.p, 0, n, 0, g->max_row, g->idx.p, g->bin.p, g->has_pix ? g->pix.p : nullptr, st);
             launches += 1;
         }
-        k_row_stats<<<blocks_for(n * 32, 256), 256, 0, st>>>(g->ptr.p, g->idx.p, 0, 0, (int32_t)n, stats.p);
-        launches += 1;
-        GR_CUDA(cudaGetLastError());
+        GR_CUDA(cudaGetLastError());      // (row statistics of the slot-table kernel: on first use, gr_row_stats)
     } else {
         g->h_idx_bytes = std::max<size_t>((size_t)E * 4 + 256, 256);
         g->h_bin_bytes = std::max<size_t>((size_t)E + 256, 256);
@@ -836,7 +872,7 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             int64_t len = w.e_hi - w.e_lo;
             int64_t s_lo = g->spatial ? w.row_lo : 0, s_hi = g->spatial ? w.row_hi : n;
             unsigned nb2 = blocks_for((s_hi - s_lo) * 32, 256);
-            k_neighbours<true><<<nb2, 256, 0, st>>>(sx.p, sy.p, sz.p, lab.p, cell_start.p, s_lo, s_hi, w.row_lo, w.row_hi,
+            k_neighbours<true><<<nb2, 256, 0, st>>>(bp, eq, sx.p, sy.p, sz.p, lab.p, cell_start.p, s_lo, s_hi, w.row_lo, w.row_hi,
                                                     nullptr, g->ptr.p, w.e_lo, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr);
             launches += 1;
             if (!g->spatial) {
@@ -864,7 +900,7 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             GR_CUDA(cudaStreamSynchronize(st));
         }
     }
-    {
+    if (g->ooc) {
         int32_t h[32];
         GR_CUDA(cudaMemcpyAsync(h, stats.p, sizeof h, cudaMemcpyDeviceToHost, st));
         GR_CUDA(cudaStreamSynchronize(st));
@@ -872,9 +908,46 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             g->max_ptl[s] = h[2 * (s - GR_S_MIN)];
             g->max_pages[s] = h[2 * (s - GR_S_MIN) + 1];
         }
+        g->stats_done = 1;
     }
+    // range of |w|: the gather kernel accumulates weighted sums in fixed point when the weights are of one scale
+    if (d_weights && n > 0) {
+        DevBuf<double> mm;
+        mm.alloc(2);
+        const double init[2] = {INFINITY, 0.0};
+        double h[2];
+        GR_CUDA(cudaMemcpyAsync(mm.p, init, 16, cudaMemcpyHostToDevice, st));
+        k_abs_minmax<<<296, 256, 0, st>>>(g->w.p, n, mm.p);
+        GR_CUDA(cudaMemcpyAsync(h, mm.p, 16, cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        g->w_absmin = h[0];
+        g->w_absmax = h[1];
+        launches += 1;
+    }
+    if (const char *e = getenv("GRAMSCI_GATHER_G")) g->algo_g = (atoi(e) == 1 || atoi(e) == 8) ? atoi(e) : 0;
     g->t_build_ms = timer.stop();
     g->n_launches = launches;
+}
+
+// row statistics of the slot-table 3pCF kernel, on first use (in-core graphs; capped graphs gather them in the build)
+void gr_row_stats(gramsci_graph *g)
+{
+    if (g->stats_done || g->ooc || g->n <= 0) return;
+    cudaStream_t st = g->stream;
+    DevBuf<int32_t> stats;
+    stats.alloc(32);
+    GR_CUDA(cudaMemsetAsync(stats.p, 0, sizeof(int32_t) * 32, st));
+    k_row_stats<<<blocks_for(g->n * 32, 256), 256, 0, st>>>(g->ptr.p, g->idx.p, 0, 0, (int32_t)g->n, stats.p);
+    GR_CUDA(cudaGetLastError());
+    int32_t h[32];
+    GR_CUDA(cudaMemcpyAsync(h, stats.p, sizeof h, cudaMemcpyDeviceToHost, st));
+    GR_CUDA(cudaStreamSynchronize(st));
+    for (int s = GR_S_MIN; s <= GR_S_MAX; ++s) {
+        g->max_ptl[s] = h[2 * (s - GR_S_MIN)];
+        g->max_pages[s] = h[2 * (s - GR_S_MIN) + 1];
+    }
+    g->stats_done = 1;
+    g->n_launches += 1;
 }
 
 // ---------------------------------------------------------------------------------------------------

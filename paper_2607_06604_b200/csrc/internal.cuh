@@ -33,20 +33,31 @@ struct GrFail { int code; };   // thrown inside the library only; every ABI entr
     } while (0)
 
 // ---- device buffer owned by the library --------------------------------------------------------
-// Stream-ordered allocations (cudaMallocAsync from the device's default pool, release threshold raised
-// so that freed blocks are reused by the next call instead of going back to the driver): a graph build
-// or a query allocates tens of scratch buffers and must not pay a device synchronisation for each.
-// Every ABI entry sets the stream its buffers are ordered on (gr_alloc_stream); all library work
-// runs on that stream.
-cudaStream_t &gr_alloc_stream();
-bool gr_pools_supported();
+// Where device memory comes from (include/gramsci.h, gramsci_options.alloc / dealloc):
+//  * the caller's allocator hooks when given (PyTorch's caching allocator in the Python binding), else
+//  * stream-ordered allocations from a PRIVATE memory pool of the device (cudaMallocFromPoolAsync; release
+//    threshold raised so that freed blocks are reused by the next call instead of going back to the driver: a
+//    graph build or a query allocates tens of scratch buffers and must not pay a device synchronisation for
+//    each).  The device's default pool is left alone; gramsci_release_memory() trims the private one.
+// Every ABI entry sets the allocation context of the calling thread (gr_alloc_ctx); all library work runs
+// on that stream.
+struct GrAllocCtx {
+    cudaStream_t stream = nullptr;
+    void *(*alloc)(size_t, void *, void *) = nullptr;
+    void (*dealloc)(void *, void *, void *) = nullptr;
+    void *user = nullptr;
+};
+GrAllocCtx &gr_alloc_ctx();
+inline cudaStream_t &gr_alloc_stream() { return gr_alloc_ctx().stream; }
+void *gr_dev_alloc(size_t bytes, const GrAllocCtx &ctx, int *kind);     // kind: 0 cudaMalloc, 1 pool, 2 hook
+void gr_dev_free(void *p, const GrAllocCtx &ctx, int kind);
 
 template <typename T>
 struct DevBuf {
     T *p = nullptr;
     size_t n = 0;
-    cudaStream_t st = nullptr;
-    bool async = false;
+    GrAllocCtx ctx;
+    int kind = 0;
     DevBuf() {}
     DevBuf(const DevBuf &) = delete;
     DevBuf &operator=(const DevBuf &) = delete;
@@ -56,16 +67,11 @@ struct DevBuf {
         n = count;
         size_t bytes = (count ? count : 1) * sizeof(T);
         bytes = (bytes + 255) & ~size_t(255);          // tail padding: aligned vector loads may over-read
-        async = gr_pools_supported();
-        st = gr_alloc_stream();
-        if (async) GR_CUDA(cudaMallocAsync((void **)&p, bytes + 256, st));
-        else GR_CUDA(cudaMalloc((void **)&p, bytes + 256));
+        ctx = gr_alloc_ctx();
+        p = (T *)gr_dev_alloc(bytes + 256, ctx, &kind);
     }
     void release() {
-        if (p) {
-            if (async) cudaFreeAsync(p, st);
-            else cudaFree(p);
-        }
+        if (p) gr_dev_free(p, ctx, kind);
         p = nullptr;
         n = 0;
     }
@@ -81,6 +87,28 @@ struct GrWindow {
 #define GR_HUB_SELECTED(v, i) (((v).hub_stride <= 1 || ((i) % (v).hub_stride) == 0) && \
                                ((v).shard_count <= 1 || ((i) % (v).shard_count) == (v).shard_index))
 
+// Dense cell-block rows (dense.cu).  Row of point j (cell c, position p = j - cell_start[c]) lives at
+// dbase[c] + p * rowlen[c] and holds, for every cell c' of the FORWARD stencil of c (the stencil cells with id >= c,
+// ascending: fwd_cell[c*27 + o], o < nf[c]) a segment of occ(c') bytes at fwd_off[c*27 + o]: byte q of the segment
+// = bin of the edge (j, cell_start[c'] + q) or 0xFF.  This is P:149's lmat idea made global: one byte answers
+// "is (j,k) an edge and in which bin" for any k > j.
+#define GR_STENCIL 27
+struct GrDense {
+    int state = 0;                 // 0 not tried, 1 built, -1 not applicable (reason in `why`)
+    const char *why = "";
+    DevBuf<int32_t> fwd_cell, fwd_off;     // [ncell*27]
+    DevBuf<int32_t> nf, rowlen;            // [ncell]
+    DevBuf<int64_t> dbase;                 // [ncell+1] byte offset of the first row of every cell
+    DevBuf<uint8_t> bytes;                 // in-core: all rows
+    DevBuf<int32_t> unit_lo;               // [n_units+1] work units: hub label ranges inside one cell
+    DevBuf<unsigned int> unit_w;           // [n_units] wedges (sum of C(len,2) over the unit's hubs), saturated
+    int n_units = 0, unit_hubs = 0;
+    unsigned long long unit_wedges = 0;
+    int64_t total = 0;
+    int32_t max_occ = 0, max_rowlen = 0;
+    double t_build_ms = 0;
+};
+
 struct gramsci_graph {
     // parameters
     int64_t n = 0;
@@ -90,7 +118,10 @@ struct gramsci_graph {
     double r_min = 0, r_max = 0;
     double q[GR_MAXBINS + 1];      // squared bin edges (A-3)
     int weighted = 0, has_pix = 0, spatial = 0, algo = 0, hub_stride = 1, shard_count = 1, shard_index = 0;
+    int algo_g = 0;                // gather kernel: forced warps per hub (test knob GRAMSCI_GATHER_G), 0 = choose
+    double w_absmin = 1.0, w_absmax = 1.0;   // range of |w| (1 for unit weights): picks fixed-point or fp64 weighted sums
     cudaStream_t stream = nullptr;
+    GrAllocCtx actx;               // allocator of this graph (hooks or the private pool), set at build
     int sm_count = GR_SM_COUNT_FALLBACK;
     size_t smem_optin = 0;
     // cell grid
@@ -105,10 +136,16 @@ struct gramsci_graph {
     DevBuf<double> w;              // [n] weights by internal label
     DevBuf<int32_t> order;         // [n] label at spatial slot s
     DevBuf<int32_t> caller_of;     // [n] caller label of internal label (spatial mode), else empty
+    // cell list kept for the dense cell-block rows (dense.cu; spatial mode): labels of cell c are
+    // [cell_start[c], cell_start[c+1]); cell_of[label] = cell id
+    DevBuf<int32_t> cell_start, cell_of;
+    int64_t ncell = 0;
+    GrDense dn;                    // dense rows + per-cell layout tables (built on first use by the gather kernel)
     // row statistics for the slot-table 3pCF kernel (query3.cu; k_row_stats in build_graph.cu): for page
     // size 2^s labels (s = GR_S_MIN .. GR_S_MAX), the longest page table and the most pages a row touches
     int32_t max_ptl[16] = {0};
     int32_t max_pages[16] = {0};
+    int stats_done = 0;
     // 4pCF: raw 6-tuple -> (canonical configuration id | chirality code << 24), and configuration id -> dense
     // index; built on the device at the first 4pCF call (query4.cu)
     DevBuf<uint32_t> lut4;
@@ -126,6 +163,12 @@ struct gramsci_graph {
     double t_build_ms = 0, t_query_ms = 0, t_enum_ms = 0, n_launches = 0, staged_bytes = 0;
 };
 
+// Hit budget after which a kernel drains its shared-memory uint32 histogram into the global uint64 one (bins must
+// not wrap).  The defaults are reached only by the largest workloads; the parity tests set the environment
+// variable GRAMSCI_FLUSH_BUDGET (read at every query) to a few thousand so that every kernel variant drains many
+// times on small inputs and is compared bin by bin with the oracle.
+unsigned long long gr_flush_budget(unsigned long long dflt);
+
 // opt the kernel in to `smem` bytes of dynamic shared memory and return its resident CTAs per SM; both driver calls
 // are cached per (device, kernel, size) -- they cost a few hundred microseconds per query otherwise (api.cu)
 int gr_kernel_occupancy(const void *fn, int threads, size_t smem);
@@ -137,6 +180,7 @@ void gr_pinned_free(void *p, size_t bytes);
 
 // ---- build_graph.cu -----------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced);
+void gr_row_stats(gramsci_graph *g);
 void gr_export_csr(const gramsci_graph *g, int64_t *d_ptr, int32_t *d_idx, uint8_t *d_bin, uint8_t *d_pix);
 void gr_exclusive_scan_i32(const int32_t *d_in, int64_t n, int32_t *d_out /*[n+1]*/, cudaStream_t st);
 
@@ -155,12 +199,30 @@ struct GrView {
     const double *w;        // weights by label or nullptr
     int32_t hub_stride;     // > 1: only hubs with label % hub_stride == 0
     int32_t shard_count, shard_index;   // shard_count > 1: only hubs with label % shard_count == shard_index
+    // dense cell-block rows of the resident search rows (gather kernel): row of label j at dense + rowaddr(j) - d0
+    const uint8_t *dense; int64_t d0;
 };
 
 void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
 void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
 void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c, double *d_even_w, double *d_odd_w);
 void gr_work_counters(gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
+
+// dense.cu: layout tables + dense rows (in-core) for the gather kernel; returns false when not applicable
+bool gr_dense_prepare(gramsci_graph *g);
+// expand the CSR rows [row_lo,row_hi) (edge arrays starting at edge e0) into dense rows at `out` (= row row_lo)
+// (`out` + rowaddr(row) - d0 is where a row lands; the first out_bytes bytes of `out` are reset to 0xFF)
+void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int32_t *idx, const uint8_t *bin, int64_t e0,
+                     uint8_t *out, int64_t d0, int64_t out_bytes, cudaStream_t st);
+void gr_dense_units(gramsci_graph *g, int max_hubs, unsigned long long max_wedges);
+int64_t gr_dense_rowaddr_host(gramsci_graph *g, int32_t row);      // byte offset of a row (reads the device tables)
+// query3g.cu: the gather 3pCF kernel as a tile function
+bool gr_gather_applicable(gramsci_graph *g, bool weighted, const char **why);
+void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilateral);
+void gr_fold3(gramsci_graph *g, int nb, const unsigned long long *raw_cnt, const double *raw_w, int n_slots,
+              uint64_t *d_counts, double *d_wsum);
+template <typename InT, typename OutT>
+void gr_exclusive_scan(const InT *d_in, int64_t n, OutT *d_out, cudaStream_t st);
 
 // tiler.cu: run `tile_fn(view)` over every needed (hub window, search window) tile
 struct GrTileRunner;

@@ -32,6 +32,8 @@ struct Q3Params {
     int smem_hist;      // 1: uint32 histogram in shared memory
     int weighted;
     int want_counts;
+    int n_slabs;        // fp64 slabs in g_w (a CTA adds to slab blockIdx % n_slabs)
+    unsigned long long flush;   // drain the shared uint32 histogram before the CTA's hit budget passes this
 };
 
 __device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31; }
@@ -65,7 +67,7 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
     const int warp = threadIdx.x >> 5, lane = lane_id();
     if (p.smem_hist)
         for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) hist[t] = 0;
-    double *my_w = WEIGHTED ? g_w + (size_t)blockIdx.x * p.nh : nullptr;
+    double *my_w = WEIGHTED ? g_w + (size_t)(blockIdx.x % p.n_slabs) * p.nh : nullptr;
     __syncthreads();
 
     for (;;) {
@@ -81,7 +83,7 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
             // uint32 histogram overflow guard: a hub adds at most n(n-1)/2 hits
             if (p.smem_hist) {
                 unsigned long long add = (unsigned long long)n * (n - 1) / 2;
-                if (budget + add > 0xF0000000ull) {
+                if (budget + add > p.flush) {
                     for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) {
                         uint32_t c = hist[t];
                         if (c) { atomicAdd(&g_cnt[t], (unsigned long long)c); hist[t] = 0; }
@@ -205,7 +207,7 @@ k_3pcf_merge(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
         mbar_init(&s_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    double *my_w = WEIGHTED ? g_w + (size_t)blockIdx.x * p.nh : nullptr;
+    double *my_w = WEIGHTED ? g_w + (size_t)(blockIdx.x % p.n_slabs) * p.nh : nullptr;
     __syncthreads();
 
     for (;;) {
@@ -218,7 +220,7 @@ k_3pcf_merge(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
         const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
         const int n = (int)(re - rb);
         if (n >= 2) {
-            if (budget + (unsigned long long)n * (n - 1) / 2 > 0xF0000000ull) {      // uint32 bins cannot wrap
+            if (budget + (unsigned long long)n * (n - 1) / 2 > p.flush) {      // uint32 bins cannot wrap
                 for (int t = threadIdx.x; t < p.nh; t += Q3_THREADS) {
                     const uint32_t c = hist[t];
                     if (c) { atomicAdd(&g_cnt[t], (unsigned long long)c); hist[t] = 0; }
@@ -353,6 +355,8 @@ struct T3Params {
     int want_counts;
     int group_bytes;    // shared memory per group (multiple of 16)
     int hub_batch;      // schedule slots fetched per atomic
+    int n_slabs;        // fp64 slabs in g_w (a CTA adds to slab blockIdx % n_slabs)
+    unsigned long long flush;   // a warp drains the CTA histogram before its own hit budget passes this
 };
 
 template <bool WEIGHTED, int G, int U>      // U = windows in flight per trip on long rows
@@ -366,7 +370,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
     extern __shared__ __align__(16) unsigned char smem[];
     // CTA: [hist u32 nh] [group 0] [group 1] ...
     uint32_t *hist = (uint32_t *)smem;
-    double *my_w = WEIGHTED ? g_w + (size_t)blockIdx.x * p.nh : nullptr;   // fp64 partials: one slab per CTA (RED.F64)
+    double *my_w = WEIGHTED ? g_w + (size_t)(blockIdx.x % p.n_slabs) * p.nh : nullptr;   // fp64 partials: a slab per CTA while the byte budget allows (RED.F64)
     const int warp = threadIdx.x >> 5, lane = lane_id();
     const int group = warp / G, gw = warp % G;
     // (plain pointer arithmetic on `smem` only: a round trip through an integer would turn every access
@@ -593,7 +597,7 @@ k_3pcf_table(GrView v, T3Params p, unsigned int *__restrict__ hub_counter,
             }
             // uint32 bins cannot wrap: any bin holds at most the hits all 8 warps added since their own last
             // flush, and a warp flushes (atomicExch, safe against concurrent adds) before it passes 2^28
-            if (budget > (1ull << 28)) {
+            if (budget > p.flush) {
                 for (int t = lane; t < p.nh; t += 32) {
                     const uint32_t c = atomicExch(&hist[t], 0u);
                     if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
@@ -772,6 +776,14 @@ void tile_work(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------
+void gr_fold3(gramsci_graph *g, int nb, const unsigned long long *raw_cnt, const double *raw_w, int n_slots,
+              uint64_t *d_counts, double *d_wsum)
+{
+    const int nh = nb * nb * nb;
+    k_fold3<<<(nh + 255) / 256, 256, 0, g->stream>>>(nb, raw_cnt, raw_w, n_slots, (unsigned long long *)d_counts, d_wsum);
+    GR_CUDA(cudaGetLastError());
+}
+
 void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
 {
     cudaStream_t st = g->stream;
@@ -783,6 +795,20 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     g->n_launches = 0;
     g->staged_bytes = 0;
     if (!d_counts && !d_wsum) { g->t_query_ms = total.stop(); return; }
+
+    // ---- gather kernel (query3g.cu): the default wherever its dense rows apply ----
+    if (g->algo == GRAMSCI_ALGO_DEFAULT || g->algo == GRAMSCI_ALGO_GATHER) {
+        const char *why = "";
+        const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
+        const bool fits = planes * (size_t)((nh + 31) & ~31) * 4 <= 96 * 1024;
+        if (fits && !g->ooc && gr_gather_applicable(g, d_wsum != nullptr, &why)) {
+            gr_3pcf_gather(g, d_counts, d_wsum, 0);
+            return;
+        }
+        if (g->algo == GRAMSCI_ALGO_GATHER)
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: the gather kernel does not apply to this graph (%s)",
+                    fits ? (g->ooc ? "device-memory cap" : why) : "nbins^3 bins do not fit in shared memory");
+    }
 
     Q3Run r;
     r.p.nb = nb; r.p.nh = nh;
@@ -797,7 +823,10 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     // rows of hundreds of entries and more stream from DRAM (the CSR no longer lives in L2): keep 8 windows in flight
     r.long_rows = (g->n > 0 && g->n_edges / g->n >= 512) ? 1 : 0;
     r.use_merge = (g->algo == GRAMSCI_ALGO_MERGEPATH) ? 1 : 0;
+    if (g->algo >= GRAMSCI_ALGO_BITMAP && g->algo <= GRAMSCI_ALGO_TABLE_G8 && g->max_row >= 65535)
+        GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table needs rows shorter than 65535 entries (longest row %d)", g->max_row);
     if (g->algo != GRAMSCI_ALGO_BSEARCH && !r.use_merge && g->max_row >= 2 && g->max_row < 65535) {
+        gr_row_stats(g);
         const size_t hist_bytes = (((size_t)nh * 4 + 15) & ~(size_t)15) + 16;
         int best_s = -1, ptl = 0, tbl = 0;
         size_t best = 0;
@@ -825,7 +854,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
                 r.smem = hist_bytes + (size_t)(Q3_WARPS / G) * r.t.group_bytes;
             }
         }
-        if (!r.use_table && g->algo >= GRAMSCI_ALGO_BITMAP)
+        if (!r.use_table && g->algo >= GRAMSCI_ALGO_BITMAP && g->algo <= GRAMSCI_ALGO_TABLE_G8)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table does not fit in shared memory (longest row %d)", g->max_row);
     }
     const void *fn;
@@ -861,7 +890,11 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     counter.alloc(1);
     raw_cnt.alloc((size_t)nh);
     GR_CUDA(cudaMemsetAsync(raw_cnt.p, 0, sizeof(unsigned long long) * nh, st));
-    const int n_slots = r.grid;                         // one fp64 slab per CTA (weighted only)
+    // fp64 slabs (weighted only): one per CTA while they fit a byte budget, else CTAs share slabs (blockIdx % n)
+    const int n_slots = (int)std::max<int64_t>(1, std::min<int64_t>(r.grid, ((int64_t)256 << 20) / ((int64_t)nh * 8)));
+    r.p.n_slabs = r.t.n_slabs = n_slots;
+    r.p.flush = gr_flush_budget(0xF0000000ull);
+    r.t.flush = gr_flush_budget(1ull << 28);
     if (W) {
         raw_w.alloc((size_t)nh * n_slots);
         GR_CUDA(cudaMemsetAsync(raw_w.p, 0, sizeof(double) * (size_t)nh * n_slots, st));
@@ -873,9 +906,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         gr_for_each_tile(g, false, false, tile_3pcf, &r);
         g->t_enum_ms = en.stop();
     }
-    k_fold3<<<(nh + 255) / 256, 256, 0, st>>>(nb, d_counts ? raw_cnt.p : nullptr, W ? raw_w.p : nullptr, n_slots,
-                                             (unsigned long long *)d_counts, d_wsum);
-    GR_CUDA(cudaGetLastError());
+    gr_fold3(g, nb, d_counts ? raw_cnt.p : nullptr, W ? raw_w.p : nullptr, n_slots, d_counts, d_wsum);
     g->n_launches += 1;
     GR_CUDA(cudaStreamSynchronize(st));
     g->t_query_ms = total.stop();

@@ -46,6 +46,7 @@ struct Q4Params {
     int parity, weighted, want_counts;
     int n_shards;
     int ncfg;            // LUT path: number of canonical configurations (histograms are indexed by configuration)
+    unsigned long long flush;   // LUT path: a warp drains the CTA histograms before its hit budget passes this
 };
 
 __constant__ int8_t c_perm4[24][4] = {
@@ -240,7 +241,7 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         auto account = [&](int nhit) {
             if (!LUT) return;
             budget += (unsigned long long)__reduce_add_sync(0xffffffffu, nhit);
-            if (budget > (1ull << 27)) {
+            if (budget > p.flush) {
                 for (int t = lane; t < p.ncfg; t += 32) {
                     if (cnt_e) { const uint32_t c = atomicExch(&h_e[t], 0u); if (c) atomicAdd(&cnt_e[t], (unsigned long long)c); }
                     if (cnt_o) { const int c = atomicExch(&h_o[t], 0); if (c) atomicAdd(&cnt_o[t], (unsigned long long)(long long)c); }
@@ -448,6 +449,7 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     p.weighted = (d_even_w || d_odd_w) ? 1 : 0;
     p.want_counts = (d_even_c || d_odd_c) ? 1 : 0;
     p.row_cap = std::max(16, (g->max_row + 15) & ~15);
+    p.flush = gr_flush_budget(1ull << 27);
     const int channels = (d_even_c ? 1 : 0) + (d_odd_c ? 1 : 0) + (d_even_w ? 1 : 0) + (d_odd_w ? 1 : 0);
     if (channels == 0) { GR_CUDA(cudaStreamSynchronize(st)); g->t_query_ms = total.stop(); return; }
     {   // raw histograms kept per launch: counts and/or weights, three sign classes each for the parity split

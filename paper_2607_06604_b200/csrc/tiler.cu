@@ -33,6 +33,8 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     v.hub_stride = g->hub_stride;
     v.shard_count = g->shard_count;
     v.shard_index = g->shard_index;
+    v.dense = g->dn.bytes.p;
+    v.d0 = 0;
     if (!g->ooc) {
         v.idx_h = v.idx_c = g->idx.p;
         v.bin_h = v.bin_c = g->bin.p;

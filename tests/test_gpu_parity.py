@@ -75,7 +75,8 @@ def test_2pcf(relabel):
     assert_weighted_close(w, ow)
 
 
-ALGOS = [gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_TABLE_G1, gr.ALGO_TABLE_G2, gr.ALGO_TABLE_G4, gr.ALGO_TABLE_G8]
+ALGOS = [gr.ALGO_DEFAULT, gr.ALGO_MERGEPATH, gr.ALGO_BSEARCH, gr.ALGO_BITMAP, gr.ALGO_TABLE_G1, gr.ALGO_TABLE_G2,
+         gr.ALGO_TABLE_G4, gr.ALGO_TABLE_G8, gr.ALGO_GATHER]
 
 
 @pytest.mark.parametrize("algo", ALGOS)
@@ -101,6 +102,118 @@ def test_3pcf_weighted(periodic, r_min, algo):
     c, w = gg.pcf3(weighted=True)
     assert np.array_equal(c, oc)
     assert_weighted_close(w, ow)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_histogram_drain_path_exact(algo, monkeypatch):
+    """The shared-memory uint32 histograms are drained into the global uint64 ones when a hit budget is passed
+    (2^28 per warp / 0xF0000000 per CTA by default: only the largest workload gets there).  With the budget forced
+    down to a few thousand hits every kernel variant drains hundreds of times on small inputs; every bin must
+    still equal the oracle's."""
+    monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", "3000")
+    cfg = cat.config1()
+    og, gg = build_both(cfg, algo=algo)
+    assert np.array_equal(gg.pcf3()[0], og.pcf3()[0])
+    cfg = cat.config2_data(seed=2102, n=8_000, L=200.0, mean_parents=80.0)
+    og, gg = build_both(cfg, algo=algo)
+    oc, ow = og.pcf3()
+    c, w = gg.pcf3(weighted=True)
+    assert c.sum() > 1e6 and np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+    cfg, oc = _bao_replica()
+    gg = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], algo=algo)
+    assert np.array_equal(gg.pcf3()[0], oc)
+
+
+def test_4pcf_lut_drain_path_exact(monkeypatch):
+    monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", "2000")
+    monkeypatch.setenv("GRAMSCI_4PCF_LUT", "1")
+    cfg = cat.config4(seed=4002, n=6000, cap_deg=7.0)
+    og, gg = build_both(cfg, want_pixels=True)
+    ec, ew, oc, ow = og.pcf4(parity=True)
+    gec, goc, gew, gow = gg.pcf4_parity(weighted=True)
+    assert ec.sum() > 10000 and np.array_equal(gec, ec) and np.array_equal(goc, oc)
+    assert_weighted_close(gew, ew)
+    assert_weighted_close(gow, ow, scale=np.abs(ew))
+
+
+def test_torch_allocator_hooks():
+    """S:8(b): gramsci_options.alloc / dealloc -- the graph and all scratch from PyTorch's caching allocator."""
+    torch = _torch()
+    cfg = small(71, n=5000, L=40.0, weighted=True, r_max=5.0, nb=5)
+    og = oracle.Graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    torch.cuda.synchronize()
+    torch.cuda.reset_peak_memory_stats()
+    before = torch.cuda.memory_allocated()
+    g = gr.gramsci_build_graph(torch.from_numpy(cfg["points"]).cuda(), torch.from_numpy(cfg["weights"]).cuda(), cfg["box"],
+                               cfg["r_min"], cfg["r_max"], cfg["nbins"], torch_allocator=True)
+    held = torch.cuda.memory_allocated() - before
+    assert held >= 5 * og.n_edges            # the CSR lives in torch's allocator
+    c, w = g.pcf3(weighted=True)
+    assert np.array_equal(c, og.pcf3()[0])
+    assert_weighted_close(w, og.pcf3()[1])
+    assert np.array_equal(g.pcf4()[0], og.pcf4()[0])
+    g.free()
+    assert torch.cuda.memory_allocated() - before < held
+    gr.gramsci_release_memory()
+
+
+def test_concurrent_builds_on_two_threads():
+    """include/gramsci.h THREADS: no process-global device state -- two host threads build and query different
+    graphs (different boxes, radii and bin counts) on their own streams at the same time."""
+    import threading
+    torch = _torch()
+    cfgs = [small(81, n=20000, L=60.0, r_max=5.0, nb=6), small(82, n=15000, L=33.0, r_min=1.0, r_max=4.0, nb=9, periodic=False)]
+    want = [oracle.Graph(c["points"], None, c["box"], c["r_min"], c["r_max"], c["nbins"]) for c in cfgs]
+    want = [(o.n_edges, o.pcf2()[0], o.pcf3()[0]) for o in want]
+    got = [None, None]
+    errs = []
+
+    def work(k):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                c = cfgs[k]
+                pts = torch.from_numpy(c["points"]).cuda()
+                res = []
+                for _ in range(6):
+                    g = gr.gramsci_build_graph(pts, None, c["box"], c["r_min"], c["r_max"], c["nbins"])
+                    res.append((g.info()["n_edges"], g.pcf2()[0], g.pcf3()[0]))
+                    g.free()
+                got[k] = res
+        except Exception as e:           # noqa: BLE001
+            errs.append(e)
+
+    th = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not errs, errs
+    for k in range(2):
+        for e, c2, c3 in got[k]:
+            assert e == want[k][0] and np.array_equal(c2, want[k][1]) and np.array_equal(c3, want[k][2])
+
+
+def test_range_errors_on_very_long_rows():
+    """GRAMSCI_ERANGE paths: a row too long for the kernel's shared-memory staging (66,000 mutually adjacent points:
+    rows of up to 65,999 entries, 2.2e9 edges).  Raised before any enumeration starts."""
+    torch = _torch()
+    if torch.cuda.mem_get_info()[0] < 40 * 2 ** 30:
+        pytest.skip("needs 40 GiB of free device memory")
+    n = 66_000
+    pts = np.random.default_rng(5).random((n, 3)) * 0.5 + 10.0
+    g = gr.gramsci_build_graph(torch.from_numpy(pts).cuda(), None, None, 0.0, 1.0, 3)
+    assert g.info()["max_row"] == n - 1 and g.info()["n_edges"] == n * (n - 1) // 2
+    assert g.pcf2()[0].sum() == n * (n - 1) // 2
+    with pytest.raises(gr.GramsciError) as e:
+        g.pcf4()
+    assert e.value.code == 2
+    for algo in (gr.ALGO_BSEARCH, gr.ALGO_MERGEPATH, gr.ALGO_BITMAP):
+        ga = gr.gramsci_build_graph(torch.from_numpy(pts).cuda(), None, None, 0.0, 1.0, 3, algo=algo)
+        with pytest.raises(gr.GramsciError) as e:
+            ga.pcf3()
+        assert e.value.code == 2
+        ga.free()
 
 
 def test_edge_cases():
@@ -169,6 +282,9 @@ def test_4pcf_parity(periodic):
     _, g2 = build_both(cfg)
     with pytest.raises(gr.GramsciError) as e:
         g2.pcf4_parity()
+    assert e.value.code == 1
+    with pytest.raises(gr.GramsciError) as e:       # pixels are oriented by caller label (A-10)
+        build_both(cfg, want_pixels=True, relabel=1)
     assert e.value.code == 1
 
 
@@ -384,9 +500,24 @@ def test_hub_stride_partial_results():
                                    relabel=2, hub_stride=7, algo=algo)
         assert np.array_equal(g.pcf3()[0], og.pcf3(hubs=(0, og.n, 7))[0])
         assert np.array_equal(g.pcf4()[0], og.pcf4(hubs=(0, og.n, 7))[0])
-    with pytest.raises(gr.GramsciError) as e:
-        gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], hub_stride=7)
-    assert e.value.code == 1
+        assert np.array_equal(g.export_labels(), np.arange(og.n))
+    # spatial (cell-order) labels: the stride applies to the INTERNAL label; the oracle sees the points in internal
+    # order (gramsci_export_labels), where its labels are the library's
+    for algo in (gr.ALGO_DEFAULT, gr.ALGO_GATHER, gr.ALGO_BITMAP, gr.ALGO_BSEARCH, gr.ALGO_MERGEPATH):
+        g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                   hub_stride=5, algo=algo)
+        lab = g.export_labels()
+        assert np.array_equal(np.sort(lab), np.arange(og.n))
+        oi = oracle.Graph(cfg["points"][lab], cfg["weights"][lab], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+        c, w = g.pcf3(weighted=True)
+        oc, ow = oi.pcf3(hubs=(0, og.n, 5))
+        assert 0 < oc.sum() < og.pcf3()[0].sum()
+        assert np.array_equal(c, oc)
+        assert_weighted_close(w, ow)
+        # the on-demand walk written for graphs too large to hold (what the full configs[4] test uses)
+        od = oracle.Graph(cfg["points"][lab], cfg["weights"][lab], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                          lists=False)
+        assert np.array_equal(od.pcf3_direct(np.arange(0, og.n, 5))[0], oc)
 
 
 def test_ddd_over_rrr_poisson_is_one():

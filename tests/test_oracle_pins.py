@@ -51,6 +51,25 @@ def test_graph_edges_match_kdtree(periodic, r_min):
         assert np.array_equal(a, c)
 
 
+@pytest.mark.parametrize("periodic", [True, False])
+def test_degrees_direct_match_kdtree(periodic):
+    """og_degrees_direct (rows found on demand from the cell list, graph built with lists=False): full degree
+    against cKDTree ball counts (a library routine), oriented degree against the row lengths of the stored CSR."""
+    pts, w, box, _, r_max, nb = small_cfg(13, n=1200, L=20.0, r_max=2.5, periodic=periodic)
+    r_min = 0.8
+    g = oracle.Graph(pts, None, box, r_min, r_max, nb)
+    gd = oracle.Graph(pts, None, box, r_min, r_max, nb, lists=False)
+    labels = np.arange(0, g.n, 7)
+    full, plus = gd.degrees_direct(labels)
+    start, idx, _, _ = g.csr()
+    assert np.array_equal(plus, np.diff(start)[labels])
+    tree = cKDTree(pts, boxsize=(box[0] if periodic else None))
+    big = tree.query_pairs(r_max, output_type="ndarray")
+    small = tree.query_pairs(r_min, output_type="ndarray")
+    deg = np.bincount(big.ravel(), minlength=g.n) - np.bincount(small.ravel(), minlength=g.n)
+    assert np.array_equal(full, deg[labels])
+
+
 def test_bin_byte_matches_sqrt_floor():
     pts, w, box, r_min, r_max, nb = small_cfg(12, n=800, L=15.0, r_min=0.5, r_max=3.0, nb=7)
     g = oracle.Graph(pts, None, box, r_min, r_max, nb)
