@@ -63,7 +63,7 @@ __global__ void k_cell_fwd(int64_t ncell, int ncx, int ncy, int ncz, int periodi
         }
     }
     const int occ = cell_start[c + 1] - cell_start[c];
-    const int rl = (off + 15) & ~15;
+    const int rl = (off + 31) & ~31;         // rows start on 32-byte sectors; row addresses fit 32 bits after >> 5
     nf[c] = m;
     rowlen[c] = rl;
     rowbytes[c] = (int64_t)occ * rl;
@@ -118,30 +118,33 @@ __global__ void k_rowaddr(const int32_t *__restrict__ rows, int nrows, int64_t n
     out[t] = dbase[c] + (int64_t)(j - cell_start[c]) * rowlen[c];
 }
 
-// ---- work units of the gather kernel: runs of hubs inside one cell, bounded in hubs and in wedges ---------------
-// pass 0 counts the units of every cell, pass 1 writes their first labels (and wedge totals) at the scanned offsets
+// ---- work units of the gather kernels: runs of hubs inside one cell ------------------------------------------
+// Only hubs whose row length lies in [len_lo, len_hi] count (the kernel skips the others): rows of up to a few hundred
+// entries go to the warp-per-hub kernel, longer ones to the CTA-per-hub kernel.  A unit closes after max_hubs
+// counted hubs.  pass 0 counts the units of every cell, pass 1 writes (first label, last label + 1) at the scanned
+// offsets.
 __global__ void k_units(int64_t ncell, const int32_t *__restrict__ cell_start, const int64_t *__restrict__ ptr,
-                        int max_hubs, unsigned long long max_wedges, int pass, const int32_t *__restrict__ unit_off,
-                        int32_t *__restrict__ unit_cnt, int32_t *__restrict__ unit_lo, unsigned int *__restrict__ unit_w)
+                        int max_hubs, int len_lo, int len_hi, int pass, const int32_t *__restrict__ unit_off,
+                        int32_t *__restrict__ unit_cnt, int2 *__restrict__ units)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncell) return;
     const int lo = cell_start[c], hi = cell_start[c + 1];
-    int nu = 0, hubs = 0, start = lo;
-    unsigned long long w = 0;
+    int nu = 0, hubs = 0, start = lo, last = lo;
     int out = pass ? unit_off[c] : 0;
     for (int i = lo; i < hi; ++i) {
-        const unsigned long long n = (unsigned long long)(ptr[i + 1] - ptr[i]);
-        const unsigned long long wi = n * (n ? n - 1 : 0) / 2;
-        if (hubs > 0 && (hubs >= max_hubs || w + wi > max_wedges)) {
-            if (pass) { unit_lo[out] = start; unit_w[out] = (unsigned int)min(w, 0xffffffffull); ++out; }
-            ++nu; hubs = 0; w = 0; start = i;
+        const int64_t n = ptr[i + 1] - ptr[i];
+        if (n < len_lo || n > len_hi) continue;
+        if (hubs >= max_hubs) {
+            if (pass) units[out++] = make_int2(start, last + 1);
+            ++nu; hubs = 0;
         }
+        if (hubs == 0) start = i;
+        last = i;
         ++hubs;
-        w += wi;
     }
     if (hubs > 0) {
-        if (pass) { unit_lo[out] = start; unit_w[out] = (unsigned int)min(w, 0xffffffffull); }
+        if (pass) units[out] = make_int2(start, last + 1);
         ++nu;
     }
     if (!pass) unit_cnt[c] = nu;
@@ -234,30 +237,28 @@ bool gr_dense_prepare(gramsci_graph *g)
     return true;
 }
 
-// work units for `max_hubs` hubs / `max_wedges` wedges per unit (cached for the last pair asked for)
-void gr_dense_units(gramsci_graph *g, int max_hubs, unsigned long long max_wedges)
+// work units of hubs with row length in [len_lo, len_hi], at most max_hubs per unit (cached per list)
+void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int len_hi)
 {
-    GrDense &d = g->dn;
-    if (d.unit_lo.p && d.unit_hubs == max_hubs && d.unit_wedges == max_wedges) return;
+    if (u.units.p && u.max_hubs == max_hubs && u.len_lo == len_lo && u.len_hi == len_hi) return;
     cudaStream_t st = g->stream;
     const int64_t nc = g->ncell;
     DevBuf<int32_t> cnt, off;
     cnt.alloc((size_t)nc);
     off.alloc((size_t)nc + 1);
-    k_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, g->ptr.p, max_hubs, max_wedges, 0, nullptr, cnt.p, nullptr, nullptr);
+    k_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, g->ptr.p, max_hubs, len_lo, len_hi, 0, nullptr, cnt.p, nullptr);
     gr_exclusive_scan<int32_t, int32_t>(cnt.p, nc, off.p, st);
     int32_t nu = 0;
     GR_CUDA(cudaMemcpyAsync(&nu, off.p + nc, 4, cudaMemcpyDeviceToHost, st));
     GR_CUDA(cudaStreamSynchronize(st));
-    d.unit_lo.alloc((size_t)nu + 1);
-    d.unit_w.alloc((size_t)nu + 1);
-    k_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, g->ptr.p, max_hubs, max_wedges, 1, off.p, nullptr, d.unit_lo.p, d.unit_w.p);
-    const int32_t n32 = (int32_t)g->n;
-    GR_CUDA(cudaMemcpyAsync(d.unit_lo.p + nu, &n32, 4, cudaMemcpyHostToDevice, st));
+    u.units.alloc((size_t)nu + 1);
+    if (nu > 0)
+        k_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, g->ptr.p, max_hubs, len_lo, len_hi, 1, off.p, nullptr, u.units.p);
     GR_CUDA(cudaGetLastError());
     GR_CUDA(cudaStreamSynchronize(st));
-    d.n_units = nu;
-    d.unit_hubs = max_hubs;
-    d.unit_wedges = max_wedges;
+    u.n = nu;
+    u.max_hubs = max_hubs;
+    u.len_lo = len_lo;
+    u.len_hi = len_hi;
     g->n_launches += 5;
 }

@@ -93,6 +93,10 @@ struct GrWindow {
 // = bin of the edge (j, cell_start[c'] + q) or 0xFF.  This is P:149's lmat idea made global: one byte answers
 // "is (j,k) an edge and in which bin" for any k > j.
 #define GR_STENCIL 27
+struct GrUnits {                           // hub label ranges [x, y) inside one cell
+    DevBuf<int2> units;
+    int n = 0, max_hubs = 0, len_lo = 0, len_hi = 0;
+};
 struct GrDense {
     int state = 0;                 // 0 not tried, 1 built, -1 not applicable (reason in `why`)
     const char *why = "";
@@ -100,10 +104,7 @@ struct GrDense {
     DevBuf<int32_t> nf, rowlen;            // [ncell]
     DevBuf<int64_t> dbase;                 // [ncell+1] byte offset of the first row of every cell
     DevBuf<uint8_t> bytes;                 // in-core: all rows
-    DevBuf<int32_t> unit_lo;               // [n_units+1] work units: hub label ranges inside one cell
-    DevBuf<unsigned int> unit_w;           // [n_units] wedges (sum of C(len,2) over the unit's hubs), saturated
-    int n_units = 0, unit_hubs = 0;
-    unsigned long long unit_wedges = 0;
+    GrUnits ua, ub;                        // work units of the warp-per-hub / CTA-per-hub gather kernels
     int64_t total = 0;
     int32_t max_occ = 0, max_rowlen = 0;
     double t_build_ms = 0;
@@ -214,10 +215,10 @@ bool gr_dense_prepare(gramsci_graph *g);
 // (`out` + rowaddr(row) - d0 is where a row lands; the first out_bytes bytes of `out` are reset to 0xFF)
 void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int32_t *idx, const uint8_t *bin, int64_t e0,
                      uint8_t *out, int64_t d0, int64_t out_bytes, cudaStream_t st);
-void gr_dense_units(gramsci_graph *g, int max_hubs, unsigned long long max_wedges);
+void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int len_hi);
 int64_t gr_dense_rowaddr_host(gramsci_graph *g, int32_t row);      // byte offset of a row (reads the device tables)
 // query3g.cu: the gather 3pCF kernel as a tile function
-bool gr_gather_applicable(gramsci_graph *g, bool weighted, const char **why);
+bool gr_gather_applicable(gramsci_graph *g, bool weighted, size_t hist_bytes, const char **why);
 void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilateral);
 void gr_fold3(gramsci_graph *g, int nb, const unsigned long long *raw_cnt, const double *raw_w, int n_slots,
               uint64_t *d_counts, double *d_wsum);

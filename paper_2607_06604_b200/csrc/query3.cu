@@ -800,14 +800,13 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     if (g->algo == GRAMSCI_ALGO_DEFAULT || g->algo == GRAMSCI_ALGO_GATHER) {
         const char *why = "";
         const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
-        const bool fits = planes * (size_t)((nh + 31) & ~31) * 4 <= 96 * 1024;
-        if (fits && !g->ooc && gr_gather_applicable(g, d_wsum != nullptr, &why)) {
+        const size_t hist_bytes = planes * (size_t)((nh + 31) & ~31) * 4;
+        if (!g->ooc && gr_gather_applicable(g, d_wsum != nullptr, hist_bytes, &why)) {
             gr_3pcf_gather(g, d_counts, d_wsum, 0);
             return;
         }
         if (g->algo == GRAMSCI_ALGO_GATHER)
-            GR_FAIL(GRAMSCI_ERANGE, "3pcf: the gather kernel does not apply to this graph (%s)",
-                    fits ? (g->ooc ? "device-memory cap" : why) : "nbins^3 bins do not fit in shared memory");
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: the gather kernel does not apply to this graph (%s)", g->ooc ? "device-memory cap" : why);
     }
 
     Q3Run r;

@@ -9,21 +9,23 @@
 // Work = sum_i C(len N+(i), 2) wedges instead of sum_(i,j) len N+(j) streamed list elements (0.63-0.75 x), one byte
 // load per wedge instead of a two-level table look-up per element, and no per-row streaming overhead.
 //
-// Mapping.  Work units are runs of hubs inside ONE cell (dense.cu), pulled by persistent CTAs from a global counter;
-// hubs of a cell share the forward stencil, so the CTA builds one 27x27 table T (segment offset of cell o_k inside a
-// row of cell o_j, -1 if o_k is not forward of o_j) per cell.  A group of G warps (G = 1 for rows up to a few
-// hundred entries, 8 beyond) stages the hub row as (position in its cell | stencil ordinal, bin) words plus, per
-// entry, the address of that entry's own dense row (it is a spoke for the later entries).  Lanes own tail entries
-// k; the loop runs over spokes j.  Rows of up to 128 entries keep the lane's entries in registers.
+// Hubs of one cell share the forward stencil (<= 27 cells, ordinal o); T[o_j][o_k] = offset of the segment of cell
+// o_k inside a dense row of cell o_j (0xFFFF if o_k is not forward of o_j) is built once per cell and worker.
+// A staged hub-row entry is (position in its cell | ordinal | bin) plus, for its role as a spoke, the address of its
+// own dense row.  Lanes own tail entries k, the loop runs over spokes j, so everything about j is warp-uniform.
+//   * k_3pcf_gather_warp: rows of 2..250 entries.  A WARP pulls a run of hubs of one cell (work unit, dense.cu),
+//     builds its own T, and needs no CTA barrier at all; the lane's entries stay in registers per block of 32.
+//   * k_3pcf_gather_cta:  longer rows.  A CTA per hub, spokes dealt to the 8 warps, tail streamed from shared memory.
 //
-// Histograms: per-CTA shared uint32 bins (ATOMS.POPC.INC), drained into global uint64 bins between units before a
-// budget could wrap them.  Weighted sums: fixed point.  w_i w_j w_k is scaled by a power of two so that
-// |x| < 2^40, rounded to the nearest integer and added as three limbs (14 + 14 + 12 signed bits) with three
-// native 32-bit shared atomics; 2^17 additions fit before a limb could overflow, units are cut at that many wedges,
-// and the drain recombines the limbs exactly (int64), converts once to fp64 and adds to the CTA's global slab.
-// Integer addition is associative, so the weighted result no longer depends on atomic order up to the (few) fp64
-// additions of the drains; the rounding error per term is <= 2^-41 of the largest product.  Graphs whose weights
-// span more than a factor 3.17 in magnitude (so that products span > 32) keep fp64 RED atomics (WMODE 2).
+// Histograms: per-CTA shared uint32 bins (ATOMS.POPC.INC), drained into global uint64 bins before a wedge budget
+// could wrap them.  Weighted sums (WMODE 1): FIXED POINT.  w_i w_j w_k is scaled by a power of two so that
+// |x| < 2^39, rounded to the nearest integer and added as three limbs (13 + 13 + 13 signed bits) with three native
+// 32-bit shared atomics; 2^18 - 2^12 additions fit before a limb word could overflow, the wedge budgets are cut
+// there, and the drain recombines the limb sums exactly (int64), converts once to fp64 and adds to a global fp64
+// slab.  Integer addition is associative: the weighted result no longer depends on atomic order except through the
+// few fp64 additions of the drains.  Rounding error per term <= 2^-40 of 2^ceil(log2 max|www|): with products
+// spanning at most a factor 32 that is <= 5.8e-11 of the smallest term (BASELINE's 1e-10).
+// Catalogues whose |w| span more than 32^(1/3) = 3.17 keep fp64 RED atomics into per-CTA global slabs (WMODE 2).
 #include "internal.cuh"
 
 #include <algorithm>
@@ -31,75 +33,391 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <type_traits>
 
 namespace {
 
 constexpr int G3_THREADS = 256;
 constexpr int G3_WARPS = G3_THREADS / 32;
-constexpr int LIMB_BITS = 14;
+constexpr int SHORT_CAP = 250;                 // longest row of the warp kernel: C(250,2) wedges < 2^15 - 2^9
+constexpr int SHORT_STAGE = 256;
+constexpr int LIMB_BITS = 13;
 constexpr unsigned LIMB_MASK = (1u << LIMB_BITS) - 1u;
-constexpr unsigned long long LIMB_MAX_ADDS = 1ull << 17;
+constexpr unsigned long long LIMB_CTA_ADDS = (1ull << 18) - (1ull << 12);   // per CTA between drains
+constexpr unsigned T_NONE = 0xffffu;
+constexpr unsigned ROW_NONE = 0xffffffffu;
 
 struct G3Params {
-    int nb, nh, nhp;        // bins, histogram entries (nb^3, or nb equilateral), words per shared plane
-    int row_cap;            // staged hub-row entries per group
+    int nb, nh, nhp;        // bins, histogram entries (nb^3; nb equilateral), words per shared plane
+    int row_cap;            // CTA kernel: staged hub-row entries
     int want_counts;
     int n_slabs;            // fp64 slabs in g_w
     int n_units;
-    unsigned long long flush;    // drain the counts before the CTA's wedge budget passes this
-    unsigned long long wflush;   // the same for the fixed-point limbs
+    int len_lo, len_hi;     // rows this launch takes
+    unsigned long long flush;    // counts: drain before the wedge budget (per warp / per CTA) passes this
+    unsigned long long wflush;   // limbs: the same
     double wscale, inv_wscale;
 };
 
 struct G3Tables {
     const int32_t *cell_start, *cell_of, *fwd_cell, *fwd_off, *nf, *rowlen;
     const int64_t *dbase;
-    const int32_t *unit_lo;
-    const unsigned int *unit_w;
+    const int2 *units;
 };
 
-template <int G>
-__device__ __forceinline__ void group_sync(int group)
+// ---- shared memory through 32-bit shared addresses (no generic-address arithmetic in the inner loops) ----------
+__device__ __forceinline__ unsigned s_addr(const void *p)
 {
-    if (G == 1) __syncwarp();
-    else if (G == G3_WARPS) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "r"(G * 32) : "memory");
+    unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("mov.u32 %0, %0;" : "+r"(a));        // opaque: kept in a register instead of being re-derived at every use
+    return a;
+}
+__device__ __forceinline__ unsigned lds_u16(unsigned a)
+{
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_v2(unsigned a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_f64(unsigned a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ unsigned sexch0(unsigned a)
+{
+    unsigned v;
+    asm volatile("atom.shared.exch.b32 %0, [%1], 0;" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+// predicated shared-memory reductions (no branch around the atomic): the hit test is part of the instruction
+template <bool EQ>
+__device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned ref)
+{
+    if (EQ) asm volatile("{\n .reg .pred q;\n setp.eq.u32 q, %1, %2;\n @q red.shared.add.u32 [%0], 1;\n}" ::"r"(a), "r"(bv), "r"(ref));
+    else asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %1, 255;\n @q red.shared.add.u32 [%0], 1;\n}" ::"r"(a), "r"(bv));
+}
+template <bool EQ>
+__device__ __forceinline__ void sred_limbs_hit(unsigned a, unsigned stride, unsigned l0, unsigned l1, unsigned l2, unsigned bv,
+                                               unsigned ref)
+{
+    if (EQ)
+        asm volatile("{\n .reg .pred q;\n .reg .u32 a1, a2;\n setp.eq.u32 q, %5, %6;\n add.u32 a1, %0, %4;\n add.u32 a2, a1, %4;\n"
+                     " @q red.shared.add.u32 [%0], %1;\n @q red.shared.add.u32 [a1], %2;\n @q red.shared.add.u32 [a2], %3;\n}"
+                     ::"r"(a), "r"(l0), "r"(l1), "r"(l2), "r"(stride), "r"(bv), "r"(ref));
+    else
+        asm volatile("{\n .reg .pred q;\n .reg .u32 a1, a2;\n setp.ne.u32 q, %5, 255;\n add.u32 a1, %0, %4;\n add.u32 a2, a1, %4;\n"
+                     " @q red.shared.add.u32 [%0], %1;\n @q red.shared.add.u32 [a1], %2;\n @q red.shared.add.u32 [a2], %3;\n}"
+                     ::"r"(a), "r"(l0), "r"(l1), "r"(l2), "r"(stride), "r"(bv));
 }
 
-// WMODE: 0 counts only, 1 weighted with fixed-point limbs in shared memory, 2 weighted with fp64 RED atomics.
-// EQ: equilateral restriction (S:8(f)-3): only wedges with b_ik == b_ij are followed, only hits with b_jk == b_ij count.
-template <int WMODE, int G, bool EQ>
-__global__ void __launch_bounds__(G3_THREADS)
-k_3pcf_gather(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit_counter,
-              unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
+// ---- per-cell tables -------------------------------------------------------------------------------------
+// forward stencil of cell c: lane o < nf keeps its cell id, and (start label, row length, first-row offset) go to shared
+__device__ __forceinline__ int load_fwd(const G3Tables &tb, int c, int nfc, int lane, int32_t *f_start, int32_t *f_rowlen,
+                                        int64_t *f_dbase)
 {
-    constexpr int NGROUPS = G3_WARPS / G;
+    int fc = -1, fs = INT_MAX, rl = 0;
+    int64_t db = 0;
+    if (lane < nfc) {
+        fc = tb.fwd_cell[(int64_t)c * GR_STENCIL + lane];
+        fs = tb.cell_start[fc];
+        rl = tb.rowlen[fc];
+        db = tb.dbase[fc];
+    }
+    f_start[lane] = fs;
+    f_rowlen[lane] = rl;
+    f_dbase[lane] = db;
+    return fc;
+}
+
+// row o_j of T: lane o_k gets the offset of its cell's segment in a dense row of cell cj (its forward list is sorted)
+__device__ __forceinline__ void build_T_row(const G3Tables &tb, int cj, int fc_lane, int lane, uint16_t *Trow)
+{
+    int L = -1, O = 0;
+    if (lane < GR_STENCIL) {
+        L = tb.fwd_cell[(int64_t)cj * GR_STENCIL + lane];
+        O = tb.fwd_off[(int64_t)cj * GR_STENCIL + lane];
+    }
+    unsigned val = T_NONE;
+#pragma unroll
+    for (int t = 0; t < GR_STENCIL; ++t) {
+        const int lt = __shfl_sync(0xffffffffu, L, t);
+        const int ot = __shfl_sync(0xffffffffu, O, t);
+        if (lt == fc_lane && lt >= 0) val = (unsigned)ot;
+    }
+    Trow[lane] = (uint16_t)val;
+}
+
+// One staged hub-row entry, in its two roles (ordinal o of its cell by binary search over the forward start labels):
+//   as a tail entry k:  kx = { position in its cell | (2 o) << 16 ,  histogram byte offset of b_ik }
+//   as a spoke j:       sp = { its own dense row (byte address >> 5, ROW_NONE if not resident) ,
+//                              64 o | (histogram byte offset of b_ij) << 11 }
+struct Entry { uint2 kx, sp; };
+template <bool EQ>
+__device__ __forceinline__ Entry make_entry(const GrView &v, int32_t k, unsigned b, unsigned nb4, unsigned nb24,
+                                            const int32_t *f_start, const int32_t *f_rowlen, const int64_t *f_dbase)
+{
+    int o = 0;
+#pragma unroll
+    for (int step = 16; step > 0; step >>= 1)
+        if (f_start[o + step] <= k) o += step;
+    const int pk = k - f_start[o];
+    Entry e;
+    e.kx = make_uint2((unsigned)pk | ((unsigned)o << 17), EQ ? b * 4u : b * nb4);
+    unsigned ra = ROW_NONE;
+    if (k >= v.c_lo && k < v.c_hi) ra = (unsigned)((f_dbase[o] + (int64_t)pk * f_rowlen[o] - v.d0) >> 5);
+    e.sp = make_uint2(ra, ((unsigned)o << 6) | ((EQ ? b * 4u : b * nb24) << 11));
+    return e;
+}
+
+// fixed-point limbs of a weight product (already scaled): x = l0 + l1 2^13 + l2 2^26, l0, l1 in [0, 2^13), l2 signed
+__device__ __forceinline__ void limbs_of(double pw, unsigned &l0, unsigned &l1, unsigned &l2)
+{
+    const long long x = __double2ll_rn(pw);
+    const unsigned lo = (unsigned)x, hi = (unsigned)(x >> 32);
+    l0 = lo & LIMB_MASK;
+    l1 = (lo >> LIMB_BITS) & LIMB_MASK;
+    l2 = __funnelshift_r(lo, hi, 2 * LIMB_BITS);
+}
+
+// ---- warp kernel: rows of len_lo..len_hi (<= SHORT_CAP) entries ---------------------------------------------
+// WMODE: 0 counts only, 1 weighted by fixed-point limbs in shared memory, 2 weighted by fp64 RED atomics.
+// EQ: equilateral restriction (S:8(f)-3): only wedges with b_ik == b_ij are followed, only hits with b_jk == b_ij count.
+// OOC: spokes whose dense row is not resident are skipped (out-of-core tiles).
+template <int WMODE, bool EQ, bool OOC>
+__global__ void __launch_bounds__(G3_THREADS)
+k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit_counter,
+                   unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
+{
     extern __shared__ __align__(16) unsigned char smem[];
-    // CTA: [hist u32 nhp (counts)] [limbs 3 x nhp (WMODE 1)] [T i32 27x32] [f_start, f_rowlen i32 32 each] [f_dbase i64 32]
-    //      then per group: [kw uint2 row_cap] [rbase i64 row_cap] [aw f64 row_cap (weighted)]
+    // CTA: [hist u32 nhp (counts)] [limbs 3 x nhp (WMODE 1)], then per warp:
+    //      [T u16 27x32] [f_start i32 32] [f_rowlen i32 32] [f_dbase i64 32] [sp uint2 cap] [kx uint2 cap] [aw f64 cap (weighted)]
     const bool have_cnt = (WMODE == 0) || p.want_counts;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t *hist = (uint32_t *)smem;
-    uint32_t *limb = hist + (have_cnt ? p.nhp : 0);
-    int32_t *T = (int32_t *)(limb + (WMODE == 1 ? 3 * p.nhp : 0));
-    int32_t *f_start = T + GR_STENCIL * 32;
+    const int planes = (have_cnt ? 1 : 0) + (WMODE == 1 ? 3 : 0);
+    const int cap = p.row_cap;
+    const size_t per_warp = GR_STENCIL * 32 * 2 + 128 + 128 + 256 + (size_t)cap * (16 + (WMODE ? 8 : 0));
+    unsigned char *ws = smem + (size_t)planes * p.nhp * 4 + (size_t)warp * per_warp;
+    uint16_t *T = (uint16_t *)ws;
+    int32_t *f_start = (int32_t *)(ws + GR_STENCIL * 32 * 2);
     int32_t *f_rowlen = f_start + 32;
     int64_t *f_dbase = (int64_t *)(f_rowlen + 32);
-    unsigned char *gs = (unsigned char *)(f_dbase + 32);
+    uint2 *sp = (uint2 *)(f_dbase + 32);
+    uint2 *kx = sp + cap;
+    double *aw = (double *)(kx + cap);
+    const unsigned a_hist = s_addr(hist), a_T = s_addr(T), a_sp = s_addr(sp), a_kx = s_addr(kx), a_aw = s_addr(aw);
+    const unsigned plane_b = (unsigned)p.nhp * 4;
+    const unsigned a_limb = a_hist + (have_cnt ? plane_b : 0u);
+
+    for (int t = threadIdx.x; t < planes * p.nhp; t += G3_THREADS) hist[t] = 0u;
+    __syncthreads();
+
+    const unsigned nb4 = (unsigned)p.nb * 4u, nb24 = (unsigned)p.nb * p.nb * 4u;
+    double *my_w = WMODE ? g_w + (size_t)(blockIdx.x % p.n_slabs) * p.nh : nullptr;
+    unsigned long long cb = 0, wb = 0;          // this warp's wedges since ITS last drain
+
+    // any warp may drain the CTA histograms (exchange with 0 is safe against the other warps' additions; the limb
+    // sums are linear, so it does not matter which drain collects which limb of a concurrent hit)
+    auto warp_drain = [&]() {
+        for (int t = lane; t < p.nh; t += 32) {
+            if (have_cnt) {
+                const unsigned c = sexch0(a_hist + 4u * t);
+                if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
+            }
+            if (WMODE == 1) {
+                const unsigned s0 = sexch0(a_limb + 4u * t), s1 = sexch0(a_limb + plane_b + 4u * t),
+                               s2 = sexch0(a_limb + 2u * plane_b + 4u * t);
+                if (s0 | s1 | s2) {
+                    const long long x = (long long)s0 + ((long long)s1 << LIMB_BITS) + ((long long)(int32_t)s2 << (2 * LIMB_BITS));
+                    atomicAdd(&my_w[t], (double)x * p.inv_wscale);
+                }
+            }
+        }
+        cb = wb = 0;
+    };
+
+    int cur_cell = -1;
+    for (;;) {
+        int u = 0;
+        if (lane == 0) u = (int)atomicAdd(unit_counter, 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= p.n_units) break;
+        const int2 un = tb.units[u];
+        if (un.y <= v.h_lo || un.x >= v.h_hi) continue;
+        const int c = tb.cell_of[un.x];
+        if (c != cur_cell) {
+            const int nfc = tb.nf[c];
+            __syncwarp();
+            const int fc = load_fwd(tb, c, nfc, lane, f_start, f_rowlen, f_dbase);
+            for (int oj = 0; oj < nfc; ++oj) build_T_row(tb, __shfl_sync(0xffffffffu, fc, oj), fc, lane, T + oj * 32);
+            cur_cell = c;
+            __syncwarp();
+        }
+        for (int i = un.x; i < un.y; ++i) {
+            const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
+            const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
+            const int n = (int)(re - rb);
+            if (n < p.len_lo || n > p.len_hi) continue;
+            const unsigned long long wedges = (unsigned long long)n * (n - 1) / 2;
+            if (cb + wedges > p.flush || (WMODE == 1 && wb + wedges > p.wflush)) warp_drain();
+            cb += wedges;
+            wb += wedges;
+            const int32_t *gi = v.idx_h + (rb - v.e0_h);
+            const uint8_t *gb = v.bin_h + (rb - v.e0_h);
+            __syncwarp();                               // the previous hub's entries are no longer read
+            for (int t = lane; t < n; t += 32) {
+                const int32_t k = gi[t];
+                const Entry e = make_entry<EQ>(v, k, gb[t], nb4, nb24, f_start, f_rowlen, f_dbase);
+                kx[t] = e.kx;
+                sp[t] = e.sp;
+                if (WMODE) aw[t] = v.w[k];
+            }
+            __syncwarp();
+            const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
+
+            // blocks of 32 tail entries (the lane's entry in registers); spokes a < min(n - 1, end of the block)
+            for (int r0 = 0; r0 < n; r0 += 32) {
+                const int t = r0 + lane;
+                // a lane without an entry looks up ordinal 31, whose T column is T_NONE for every spoke
+                const uint2 kxv = (t < n) ? lds_v2(a_kx + 8u * t) : make_uint2(31u << 17, 0u);
+                const unsigned pk = kxv.x & 0xffffu;
+                const unsigned a_Tk = a_T + (kxv.x >> 16);
+                const unsigned a_hk = (EQ ? a_hist : a_hist + kxv.y);     // counts plane; limb planes follow at plane_b strides
+                const double ak = (WMODE && t < n) ? lds_f64(a_aw + 8u * t) : 0.0;
+                const int a_end = min(n - 1, r0 + 31);
+                // U spokes at a time: all loads of a stage before the next stage.  TRI: spokes inside the lane's own block
+                // (a >= r0) need the test t > a; BOUND: a partial chunk at the end of a range
+                auto chunk = [&](int a0, auto Uc, auto TRIc, int lim) {
+                    constexpr int U = decltype(Uc)::value;
+                    constexpr bool TRI = decltype(TRIc)::value;
+                    uint2 s[U];
+                    unsigned off[U], bv[U];
+                    double wa[U];
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        s[q] = lds_v2(a_sp + 8u * (a0 + q));
+                        if (WMODE) wa[q] = lds_f64(a_aw + 8u * (a0 + q));
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        off[q] = T_NONE;
+                        if (!OOC || s[q].x != ROW_NONE) off[q] = lds_u16(a_Tk + (s[q].y & 0x7c0u));
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        bool act = off[q] != T_NONE;
+                        if (TRI) act = act && t > a0 + q;
+                        if (EQ) act = act && kxv.y == (s[q].y >> 11);
+                        bv[q] = 0xffu;
+                        if (act) bv[q] = __ldg(v.dense + ((size_t)s[q].x << 5) + (off[q] + pk));
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const unsigned hb = s[q].y >> 11;                // byte offset of b_ij in the histogram (EQ: 4 b_ij)
+                        const unsigned ah = EQ ? a_hist + hb : a_hk + hb + bv[q] * 4u;
+                        if (have_cnt) sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
+                        if (WMODE == 1) {
+                            unsigned l0, l1, l2;
+                            limbs_of((wi * wa[q]) * ak, l0, l1, l2);
+                            sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], hb >> 2);
+                        } else if (WMODE == 2) {
+                            if (EQ ? (bv[q] == (hb >> 2)) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], (wi * wa[q]) * ak);
+                        }
+                    }
+                    (void)lim;
+                };
+                using U4 = std::integral_constant<int, 4>;
+                using U1 = std::integral_constant<int, 1>;
+                const int a_mid = min(a_end, r0);                        // spokes before the block: every lane's entry is beyond them
+                int a = 0;
+                for (; a + 4 <= a_mid; a += 4) chunk(a, U4(), std::false_type(), 0);
+                for (; a < a_mid; ++a) chunk(a, U1(), std::false_type(), 0);
+                for (; a + 4 <= a_end; a += 4) chunk(a, U4(), std::true_type(), 0);
+                for (; a < a_end; ++a) chunk(a, U1(), std::true_type(), 0);
+            }
+        }
+    }
+    __syncthreads();
+    // final drain, cooperative
+    for (int t = threadIdx.x; t < p.nh; t += G3_THREADS) {
+        if (have_cnt) {
+            const uint32_t c = hist[t];
+            if (c) atomicAdd(&g_cnt[t], (unsigned long long)c);
+        }
+        if (WMODE == 1) {
+            const uint32_t *limb = hist + (have_cnt ? p.nhp : 0);
+            const uint32_t s0 = limb[t], s1 = limb[p.nhp + t], s2 = limb[2 * p.nhp + t];
+            if (s0 | s1 | s2) {
+                const long long x = (long long)s0 + ((long long)s1 << LIMB_BITS) + ((long long)(int32_t)s2 << (2 * LIMB_BITS));
+                atomicAdd(&my_w[t], (double)x * p.inv_wscale);
+            }
+        }
+    }
+}
+
+// ---- CTA kernel: rows longer than the warp kernel takes; one hub per CTA at a time -------------------------------
+// Rows of thousands of entries: 4 bytes of shared memory per staged entry (position in cell | ordinal << 16 |
+// bin << 21) so that several CTAs fit an SM; what a spoke needs (its dense row, its row of T, its histogram offset)
+// is derived once per spoke from its entry.  T holds 32-bit offsets here (dense rows of long-row graphs pass 64 KB).
+__device__ __forceinline__ unsigned lds_u32(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+
+__device__ __forceinline__ void build_T_row32(const G3Tables &tb, int cj, int fc_lane, int lane, uint32_t *Trow)
+{
+    int L = -1, O = 0;
+    if (lane < GR_STENCIL) {
+        L = tb.fwd_cell[(int64_t)cj * GR_STENCIL + lane];
+        O = tb.fwd_off[(int64_t)cj * GR_STENCIL + lane];
+    }
+    unsigned val = ROW_NONE;
+#pragma unroll
+    for (int t = 0; t < GR_STENCIL; ++t) {
+        const int lt = __shfl_sync(0xffffffffu, L, t);
+        const int ot = __shfl_sync(0xffffffffu, O, t);
+        if (lt == fc_lane && lt >= 0) val = (unsigned)ot;
+    }
+    Trow[lane] = val;
+}
+
+template <int WMODE, bool EQ, bool OOC>
+__global__ void __launch_bounds__(G3_THREADS)
+k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit_counter,
+                  unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    // [hist u32 nhp (counts)] [limbs 3 x nhp (WMODE 1)] [T u32 27x32] [f_start, f_rowlen i32 32 each] [f_dbase i64 32]
+    // [aw f64 row_cap (weighted)] [kx u32 row_cap]
+    const bool have_cnt = (WMODE == 0) || p.want_counts;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int group = warp / G, gw = warp % G;
-    const size_t per_entry = 16 + (WMODE ? 8 : 0);
-    gs += (size_t)group * p.row_cap * per_entry;
-    uint2 *kw = (uint2 *)gs;
-    int64_t *rbase = (int64_t *)(kw + p.row_cap);
-    double *aw = (double *)(rbase + p.row_cap);
+    uint32_t *hist = (uint32_t *)smem;
+    const int planes = (have_cnt ? 1 : 0) + (WMODE == 1 ? 3 : 0);
+    uint32_t *limb = hist + (have_cnt ? p.nhp : 0);
+    uint32_t *T = hist + (size_t)planes * p.nhp;
+    int32_t *f_start = (int32_t *)(T + GR_STENCIL * 32);
+    int32_t *f_rowlen = f_start + 32;
+    int64_t *f_dbase = (int64_t *)(f_rowlen + 32);
+    double *aw = (double *)(f_dbase + 32);
+    uint32_t *kx = (uint32_t *)(aw + (WMODE ? p.row_cap : 0));
+    const unsigned a_hist = s_addr(hist), a_T = s_addr(T), a_kx = s_addr(kx), a_aw = s_addr(aw);
+    const unsigned plane_b = (unsigned)p.nhp * 4;
     __shared__ int s_unit;
 
-    const int nb = p.nb, nb2 = nb * nb;
+    for (int t = threadIdx.x; t < planes * p.nhp; t += G3_THREADS) hist[t] = 0u;
+    const unsigned nb4 = (unsigned)p.nb * 4u, nb24 = (unsigned)p.nb * p.nb * 4u;
     double *my_w = WMODE ? g_w + (size_t)(blockIdx.x % p.n_slabs) * p.nh : nullptr;
-    for (int t = threadIdx.x; t < (have_cnt ? p.nhp : 0) + (WMODE == 1 ? 3 * p.nhp : 0); t += G3_THREADS) hist[t] = 0u;
 
-    // cooperative drain of the shared histograms (all threads; callers synchronise before and after)
-    auto drain = [&]() {
+    auto drain = [&]() {                          // cooperative; callers synchronise before and after
         for (int t = threadIdx.x; t < p.nh; t += G3_THREADS) {
             if (have_cnt) {
                 const uint32_t c = hist[t];
@@ -115,164 +433,105 @@ k_3pcf_gather(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit
             }
         }
     };
-    // one hit: counts and weights.  key = raw histogram index; pw = w_i w_j w_k (already times the fixed-point scale, WMODE 1)
-    auto record = [&](int key, double pw) {
-        if (have_cnt) atomicAdd(&hist[key], 1u);
-        if (WMODE == 1) {
-            const long long x = __double2ll_rn(pw);
-            atomicAdd(&limb[key], (uint32_t)x & LIMB_MASK);
-            atomicAdd(&limb[p.nhp + key], (uint32_t)(x >> LIMB_BITS) & LIMB_MASK);
-            atomicAdd(&limb[2 * p.nhp + key], (uint32_t)(int32_t)(x >> (2 * LIMB_BITS)));
-        } else if (WMODE == 2) {
-            atomicAdd(&my_w[key], pw);
-        }
-    };
 
     int cur_cell = -1;
-    unsigned long long cbudget = 0, wbudget = 0;       // CTA-uniform: wedges since the last drain
+    unsigned long long cb = 0, wb = 0;            // CTA-uniform: wedges since the last drain
     for (;;) {
-        __syncthreads();
+        __syncthreads();                          // the previous unit is done: tables and staged row may be rewritten
         if (threadIdx.x == 0) s_unit = (int)atomicAdd(unit_counter, 1u);
         __syncthreads();
         const int u = s_unit;
         if (u >= p.n_units) break;
-        const int lo = tb.unit_lo[u], hi = tb.unit_lo[u + 1];
-        if (hi <= v.h_lo || lo >= v.h_hi) continue;
-        const unsigned long long uw = tb.unit_w[u];
-        if (cbudget + uw > p.flush || (WMODE == 1 && wbudget + uw > p.wflush)) {
-            drain();
-            cbudget = wbudget = 0;
-        }
-        cbudget += uw;
-        wbudget += uw;
-        const int c = tb.cell_of[lo];
-        const int nfc = tb.nf[c];
+        const int2 un = tb.units[u];
+        if (un.y <= v.h_lo || un.x >= v.h_hi) continue;
+        const int c = tb.cell_of[un.x];
         if (c != cur_cell) {
-            // ---- forward stencil of the cell and the table T[o_j][o_k] ----
-            if (threadIdx.x < 32) {
-                const int o = threadIdx.x;
-                int fs = INT_MAX, rl = 0;
-                int64_t db = 0;
-                if (o < nfc) {
-                    const int fc = tb.fwd_cell[(int64_t)c * GR_STENCIL + o];
-                    fs = tb.cell_start[fc];
-                    rl = tb.rowlen[fc];
-                    db = tb.dbase[fc];
-                }
-                f_start[o] = fs; f_rowlen[o] = rl; f_dbase[o] = db;
-            }
-            for (int x = threadIdx.x; x < GR_STENCIL * 32; x += G3_THREADS) {
-                const int oj = x >> 5, ok = x & 31;
-                int val = -1;
-                if (oj < nfc && ok < nfc && ok >= oj) {
-                    const int cj = tb.fwd_cell[(int64_t)c * GR_STENCIL + oj], ck = tb.fwd_cell[(int64_t)c * GR_STENCIL + ok];
-                    const int m = tb.nf[cj];
-                    for (int t = 0; t < m; ++t) {
-                        const int cc = tb.fwd_cell[(int64_t)cj * GR_STENCIL + t];
-                        if (cc == ck) { val = tb.fwd_off[(int64_t)cj * GR_STENCIL + t]; break; }
-                        if (cc > ck) break;
-                    }
-                }
-                T[x] = val;
-            }
+            const int nfc = tb.nf[c];
+            const int fc = load_fwd(tb, c, nfc, lane, f_start, f_rowlen, f_dbase);      // every warp writes the same values
+            for (int oj = warp; oj < nfc; oj += G3_WARPS) build_T_row32(tb, __shfl_sync(0xffffffffu, fc, oj), fc, lane, T + oj * 32);
             cur_cell = c;
+            __syncthreads();
         }
-        __syncthreads();
-
-        for (int i = lo + group; i < hi; i += NGROUPS) {
+        for (int i = un.x; i < un.y; ++i) {
             const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
             const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
             const int n = (int)(re - rb);
-            if (n < 2) continue;
+            if (n < p.len_lo || n > p.len_hi) continue;
+            const unsigned long long wedges = (unsigned long long)n * (n - 1) / 2;
+            __syncthreads();                      // the previous hub's entries are no longer read
+            if (cb + wedges > p.flush || (WMODE == 1 && wb + wedges > p.wflush)) {
+                drain();
+                cb = wb = 0;
+            }
+            cb += wedges;
+            wb += wedges;
             const int32_t *gi = v.idx_h + (rb - v.e0_h);
             const uint8_t *gb = v.bin_h + (rb - v.e0_h);
-            group_sync<G>(group);                       // the previous hub's entries are no longer read
-            for (int t = gw * 32 + lane; t < n; t += G * 32) {
+            for (int t = threadIdx.x; t < n; t += G3_THREADS) {
                 const int32_t k = gi[t];
-                const int b = gb[t];
-                int o = 0;                               // ordinal of k's cell in the forward stencil: last f_start <= k
+                int o = 0;
 #pragma unroll
                 for (int step = 16; step > 0; step >>= 1)
                     if (f_start[o + step] <= k) o += step;
-                const int pk = k - f_start[o];
-                kw[t] = make_uint2((unsigned)pk | ((unsigned)o << 16), EQ ? (unsigned)b : (unsigned)(b * nb));
-                // k as a spoke: its own dense row, if that row is resident (out-of-core: search window)
-                int64_t ra = -1;
-                if (k >= v.c_lo && k < v.c_hi) ra = f_dbase[o] + (int64_t)pk * f_rowlen[o] - v.d0;
-                rbase[t] = ra;
+                kx[t] = (unsigned)(k - f_start[o]) | ((unsigned)o << 16) | ((unsigned)gb[t] << 21);
                 if (WMODE) aw[t] = v.w[k];
             }
-            group_sync<G>(group);
+            __syncthreads();
             const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
-
-            if (G == 1 && n <= 128) {
-                // ---- short rows: the lane's tail entries live in registers; loop over spokes ----
-                constexpr int R = 4;
-                uint2 wk[R];
-                double ak[R];
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const int t = r * 32 + lane;
-                    wk[r] = (t < n) ? kw[t] : make_uint2(0u, 0u);
-                    ak[r] = (WMODE && t < n) ? aw[t] : 0.0;
-                }
-                const int nr = (n + 31) >> 5;
-#pragma unroll 2
-                for (int a = 0; a < n - 1; ++a) {
-                    const int64_t ra = rbase[a];
-                    if (ra < 0) continue;
-                    const uint2 wa = kw[a];
-                    const int32_t *Trow = T + (wa.x >> 16) * 32;
-                    const uint8_t *row = v.dense + ra;
-                    const int hb = EQ ? (int)wa.y : (int)wa.y * nb;
-                    const double wia = WMODE ? wi * aw[a] : 0.0;
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        if (r >= nr || r * 32 + 31 <= a) continue;        // warp-uniform
-                        const int t = r * 32 + lane;
-                        bool act = t > a && t < n;
-                        if (EQ) act = act && wk[r].y == wa.y;
-                        int off = -1;
-                        if (act) off = Trow[wk[r].x >> 16];
-                        if (off >= 0) {
-                            const unsigned bv = row[off + (int)(wk[r].x & 0xffffu)];
-                            if (EQ ? (bv == wa.y) : (bv != 0xffu))
-                                record(EQ ? hb : hb + (int)wk[r].y + (int)bv, WMODE ? wia * ak[r] : 0.0);
-                        }
+            unsigned long long hbud = 0;          // WMODE 1: wedges of this hub since the last drain (rows beyond 724 entries)
+            for (int a0 = 0; a0 < n - 1; a0 += G3_WARPS) {
+                if (WMODE == 1 && wedges > p.wflush) {
+                    hbud += (unsigned long long)G3_WARPS * (unsigned long long)(n - a0);
+                    if (hbud > p.wflush) {
+                        __syncthreads();
+                        drain();
+                        __syncthreads();
+                        hbud = (unsigned long long)G3_WARPS * (unsigned long long)(n - a0);
                     }
                 }
-            } else {
-                // ---- general rows: spokes dealt to the group's warps, lanes stream the tail from shared memory ----
-                unsigned long long hbudget = 0;          // G == 8, WMODE 1: wedges of this hub since the last drain
-                for (int a0 = 0; a0 < n - 1; a0 += G) {
-                    const int a = a0 + gw;
-                    if (WMODE == 1 && G == G3_WARPS) {    // rows beyond 512 entries: drain inside the hub (group == CTA)
-                        hbudget += (unsigned long long)G * (unsigned long long)(n - a0);
-                        if (hbudget > p.wflush) {
-                            __syncthreads();
-                            drain();
-                            __syncthreads();
-                            hbudget = (unsigned long long)G * (unsigned long long)(n - a0);
-                            cbudget = wbudget = 0;
-                        }
+                const int a = a0 + warp;
+                if (a >= n - 1) continue;
+                // ---- the spoke (warp-uniform) ----
+                const unsigned ea = lds_u32(a_kx + 4u * a);
+                const int oj = (ea >> 16) & 31, pj = ea & 0xffffu;
+                const unsigned ba = ea >> 21;
+                if (OOC) {
+                    const int32_t j = f_start[oj] + pj;
+                    if (j < v.c_lo || j >= v.c_hi) continue;            // its dense row is not resident
+                }
+                const uint8_t *row = v.dense + (f_dbase[oj] + (int64_t)pj * f_rowlen[oj] - v.d0);
+                const unsigned a_Tj = a_T + (unsigned)oj * 128u;
+                const unsigned a_hj = EQ ? a_hist + ba * 4u : a_hist + ba * nb24;
+                const double wia = WMODE ? wi * lds_f64(a_aw + 8u * a) : 0.0;
+                constexpr int U = 4;
+                for (int t0 = a + 1; t0 < n; t0 += 32 * U) {
+                    unsigned kk[U], off[U], bv[U];
+                    double wk[U];
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const int t = t0 + 32 * q + lane;
+                        kk[q] = (t < n) ? lds_u32(a_kx + 4u * t) : (31u << 16);
+                        if (WMODE) wk[q] = (t < n) ? lds_f64(a_aw + 8u * t) : 0.0;
                     }
-                    if (a >= n - 1) continue;
-                    const int64_t ra = rbase[a];
-                    if (ra < 0) continue;
-                    const uint2 wa = kw[a];
-                    const int32_t *Trow = T + (wa.x >> 16) * 32;
-                    const uint8_t *row = v.dense + ra;
-                    const int hb = EQ ? (int)wa.y : (int)wa.y * nb;
-                    const double wia = WMODE ? wi * aw[a] : 0.0;
-#pragma unroll 4
-                    for (int t = a + 1 + lane; t < n; t += 32) {
-                        const uint2 w = kw[t];
-                        if (EQ && w.y != wa.y) continue;
-                        const int off = Trow[w.x >> 16];
-                        if (off >= 0) {
-                            const unsigned bv = row[off + (int)(w.x & 0xffffu)];
-                            if (EQ ? (bv == wa.y) : (bv != 0xffu))
-                                record(EQ ? hb : hb + (int)w.y + (int)bv, WMODE ? wia * aw[t] : 0.0);
+#pragma unroll
+                    for (int q = 0; q < U; ++q) off[q] = lds_u32(a_Tj + ((kk[q] >> 14) & 0x7cu));
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        bool act = off[q] != ROW_NONE;
+                        if (EQ) act = act && (kk[q] >> 21) == ba;
+                        bv[q] = 0xffu;
+                        if (act) bv[q] = __ldg(row + (off[q] + (kk[q] & 0xffffu)));
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const unsigned ah = EQ ? a_hj : a_hj + (kk[q] >> 21) * nb4 + bv[q] * 4u;
+                        if (have_cnt) sred_inc_hit<EQ>(ah, bv[q], ba);
+                        if (WMODE == 1) {
+                            unsigned l0, l1, l2;
+                            limbs_of(wia * wk[q], l0, l1, l2);
+                            sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], ba);
+                        } else if (WMODE == 2) {
+                            if (EQ ? (bv[q] == ba) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], wia * wk[q]);
                         }
                     }
                 }
@@ -283,52 +542,44 @@ k_3pcf_gather(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit
     drain();
 }
 
+typedef void (*gather_kernel_t)(GrView, G3Params, G3Tables, unsigned int *, unsigned long long *, double *);
+
 struct G3Run {
     G3Params p;
     G3Tables tb;
     unsigned int *counter;
     unsigned long long *raw_cnt;
     double *raw_w;
-    int grid, G, wmode, eq;
+    int grid, wmode, eq, cta;
     size_t smem;
+    gather_kernel_t fn;
 };
 
 template <int WMODE, bool EQ>
-const void *gather_fn(int G)
+gather_kernel_t gather_fn2(int cta, int ooc)
 {
-    return G == 1 ? (const void *)k_3pcf_gather<WMODE, 1, EQ> : (const void *)k_3pcf_gather<WMODE, 8, EQ>;
+    if (cta) return ooc ? k_3pcf_gather_cta<WMODE, EQ, true> : k_3pcf_gather_cta<WMODE, EQ, false>;
+    return ooc ? k_3pcf_gather_warp<WMODE, EQ, true> : k_3pcf_gather_warp<WMODE, EQ, false>;
 }
 
-const void *gather_fn(int wmode, int G, int eq)
+gather_kernel_t gather_fn(int wmode, int eq, int cta, int ooc)
 {
-    if (eq) return wmode == 0 ? gather_fn<0, true>(G) : wmode == 1 ? gather_fn<1, true>(G) : gather_fn<2, true>(G);
-    return wmode == 0 ? gather_fn<0, false>(G) : wmode == 1 ? gather_fn<1, false>(G) : gather_fn<2, false>(G);
+    if (eq) return wmode == 0 ? gather_fn2<0, true>(cta, ooc) : wmode == 1 ? gather_fn2<1, true>(cta, ooc) : gather_fn2<2, true>(cta, ooc);
+    return wmode == 0 ? gather_fn2<0, false>(cta, ooc) : wmode == 1 ? gather_fn2<1, false>(cta, ooc) : gather_fn2<2, false>(cta, ooc);
 }
 
-template <int WMODE, bool EQ>
-void launch_gather(const G3Run *r, const GrView &v, cudaStream_t st)
-{
-    if (r->G == 1)
-        k_3pcf_gather<WMODE, 1, EQ><<<r->grid, G3_THREADS, r->smem, st>>>(v, r->p, r->tb, r->counter, r->raw_cnt, r->raw_w);
-    else
-        k_3pcf_gather<WMODE, 8, EQ><<<r->grid, G3_THREADS, r->smem, st>>>(v, r->p, r->tb, r->counter, r->raw_cnt, r->raw_w);
-}
-
+// one tile = up to two launches: the warp kernel over the short rows, the CTA kernel over the long ones
 void tile_3pcf_gather(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st)
 {
-    G3Run *r = (G3Run *)user;
-    GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
-    if (r->eq) {
-        if (r->wmode == 0) launch_gather<0, true>(r, v, st);
-        else if (r->wmode == 1) launch_gather<1, true>(r, v, st);
-        else launch_gather<2, true>(r, v, st);
-    } else {
-        if (r->wmode == 0) launch_gather<0, false>(r, v, st);
-        else if (r->wmode == 1) launch_gather<1, false>(r, v, st);
-        else launch_gather<2, false>(r, v, st);
+    G3Run *runs = (G3Run *)user;
+    for (int k = 0; k < 2; ++k) {
+        G3Run *r = &runs[k];
+        if (r->p.n_units == 0) continue;
+        GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
+        r->fn<<<r->grid, G3_THREADS, r->smem, st>>>(v, r->p, r->tb, r->counter, r->raw_cnt, r->raw_w);
+        GR_CUDA(cudaGetLastError());
+        g->n_launches += 1;
     }
-    GR_CUDA(cudaGetLastError());
-    g->n_launches += 1;
 }
 
 __global__ void k_copy_eq(int nb, const unsigned long long *__restrict__ cnt, const double *__restrict__ w, int n_slabs,
@@ -346,17 +597,23 @@ __global__ void k_copy_eq(int nb, const unsigned long long *__restrict__ cnt, co
 
 }  // namespace
 
-// Can this graph take the gather kernel?  (spatial labels, dense rows built or buildable, rows that fit the staging)
-bool gr_gather_applicable(gramsci_graph *g, bool weighted, const char **why)
+// Can this graph take the gather kernels?  (spatial labels, dense rows built or buildable, rows that fit the staging)
+bool gr_gather_applicable(gramsci_graph *g, bool weighted, size_t hist_bytes, const char **why)
 {
     static const char *none = "";
     if (why) *why = none;
-    if (!gr_dense_prepare(g)) { if (why) *why = g->dn.why; return false; }
     const size_t per_entry = 16 + (weighted ? 8 : 0);
-    if ((size_t)std::max(16, (g->max_row + 15) & ~15) * per_entry + 64 * 1024 > g->smem_optin) {
+    const size_t tables = GR_STENCIL * 32 * 2 + 128 + 128 + 256;
+    const size_t stage = (size_t)std::min(SHORT_STAGE, (g->max_row + 15) & ~15);
+    if (hist_bytes + (size_t)G3_WARPS * (tables + stage * per_entry) > g->smem_optin) {
+        if (why) *why = "the histogram does not fit in shared memory";
+        return false;
+    }
+    if (g->max_row > 125 && hist_bytes + tables + 2048 + (size_t)((g->max_row + 15) & ~15) * (4 + (weighted ? 8 : 0)) + 64 > g->smem_optin) {
         if (why) *why = "longest row does not fit the shared-memory staging of the gather kernel";
         return false;
     }
+    if (!gr_dense_prepare(g)) { if (why) *why = g->dn.why; return false; }
     return true;
 }
 
@@ -366,72 +623,91 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
     const int nb = g->nb;
     const int nh = equilateral ? nb : nb * nb * nb;
     GrTimer total(st);
-    G3Run r;
-    r.eq = equilateral ? 1 : 0;
     const bool W = d_wsum != nullptr;
-    r.p.nb = nb; r.p.nh = nh; r.p.nhp = (nh + 31) & ~31;
-    r.p.want_counts = d_counts ? 1 : 0;
-    r.p.row_cap = std::max(16, (g->max_row + 15) & ~15);
-    // weights: fixed-point limbs when the products span a factor <= 32 (error <= 2^-41 x 32 of a term), else fp64 RED
-    r.wmode = 0;
-    r.p.wscale = r.p.inv_wscale = 1.0;
+    G3Params p;
+    p.nb = nb; p.nh = nh; p.nhp = (nh + 31) & ~31;
+    p.want_counts = d_counts ? 1 : 0;
+    p.row_cap = std::max(16, (g->max_row + 15) & ~15);
+    // weights: fixed-point limbs when the products span a factor <= 32, else fp64 RED
+    int wmode = 0;
+    p.wscale = p.inv_wscale = 1.0;
     if (W) {
         const double hi = g->w_absmax, lo = g->w_absmin;
-        const char *force = getenv("GRAMSCI_WMODE");
-        r.wmode = (lo > 0.0 && hi / lo <= 3.1748 && std::isfinite(hi)) ? 1 : 2;
-        if (force && (force[0] == '1' || force[0] == '2') && !(force[0] == '1' && !(lo > 0.0))) r.wmode = force[0] - '0';
-        if (r.wmode == 1) {
+        wmode = (lo > 0.0 && std::isfinite(hi) && hi / lo <= 3.1748) ? 1 : 2;
+        if (const char *force = getenv("GRAMSCI_WMODE"))
+            if (force[0] == '2' || (force[0] == '1' && lo > 0.0 && std::isfinite(hi))) wmode = force[0] - '0';
+        if (wmode == 1) {
             int e = 0;
             std::frexp(hi * hi * hi, &e);                  // hi^3 < 2^e
-            r.p.wscale = std::ldexp(1.0, 39 - e);          // |x| < 2^39 (+ rounding)
-            r.p.inv_wscale = std::ldexp(1.0, e - 39);
+            p.wscale = std::ldexp(1.0, 39 - e);            // |x| < 2^39
+            p.inv_wscale = std::ldexp(1.0, e - 39);
         }
     }
-    const size_t per_entry = 16 + (r.wmode ? 8 : 0);
-    const size_t planes = (size_t)((r.wmode == 0 || d_counts) ? 1 : 0) + (r.wmode == 1 ? 3 : 0);
-    const size_t fixed = planes * r.p.nhp * 4 + GR_STENCIL * 32 * 4 + 32 * 4 * 2 + 32 * 8 + 64;
-    // G = 1 (a warp per hub, 8 hubs per CTA) while the rows are short; the limbs need rows <= 512 there
-    const size_t g1 = fixed + (size_t)G3_WARPS * r.p.row_cap * per_entry;
-    r.G = (g1 <= 100 * 1024 && !(r.wmode == 1 && g->max_row > 512) && g->max_row <= 1024) ? 1 : 8;
-    if (g->algo_g) r.G = g->algo_g;
-    r.smem = fixed + (size_t)(G3_WARPS / r.G) * r.p.row_cap * per_entry;
-    if (r.smem > g->smem_optin || planes * r.p.nhp * 4 > 160 * 1024)
-        GR_FAIL(GRAMSCI_ERANGE, "3pcf (gather): histogram or longest row (%d entries) does not fit in shared memory", g->max_row);
-    const void *fn = gather_fn(r.wmode, r.G, r.eq);
-    int occ = gr_kernel_occupancy(fn, G3_THREADS, r.smem);
-    occ = std::max(1, std::min(occ, 8));
-    r.grid = g->sm_count * occ;
+    const size_t planes = (size_t)((wmode == 0 || d_counts) ? 1 : 0) + (wmode == 1 ? 3 : 0);
+    const size_t hist_bytes = planes * p.nhp * 4;
+    const size_t tables = GR_STENCIL * 32 * 2 + 128 + 128 + 256, tables_cta = GR_STENCIL * 32 * 4 + 128 + 128 + 256;
 
-    r.p.flush = gr_flush_budget(0xE0000000ull);
-    r.p.wflush = std::min<unsigned long long>(LIMB_MAX_ADDS, gr_flush_budget(LIMB_MAX_ADDS));
-    // units: up to 4 hubs per group while rows are short, one hub per CTA when a CTA shares a hub
-    const int unit_hubs = (r.G == 1) ? 32 : 2;
-    gr_dense_units(g, unit_hubs, r.wmode == 1 ? r.p.wflush : 0xC0000000ull);
-    r.p.n_units = g->dn.n_units;
+    G3Run runs[2];
     GrDense &d = g->dn;
-    r.tb.cell_start = g->cell_start.p; r.tb.cell_of = g->cell_of.p; r.tb.fwd_cell = d.fwd_cell.p; r.tb.fwd_off = d.fwd_off.p;
-    r.tb.nf = d.nf.p; r.tb.rowlen = d.rowlen.p; r.tb.dbase = d.dbase.p; r.tb.unit_lo = d.unit_lo.p; r.tb.unit_w = d.unit_w.p;
-
-    if (getenv("GRAMSCI_DEBUG"))
-        fprintf(stderr, "[gramsci] 3pcf gather: G=%d wmode=%d eq=%d smem=%zu occ=%d grid=%d units=%d row=%d dense=%.3f GB (%.2f ms)\n",
-                r.G, r.wmode, r.eq, r.smem, occ, r.grid, r.p.n_units, g->max_row, d.total * 1e-9, d.t_build_ms);
-
     DevBuf<unsigned int> counter;
+    counter.alloc(2);
+    const unsigned long long cflush = gr_flush_budget(0xE0000000ull);
+    for (int k = 0; k < 2; ++k) {
+        G3Run &r = runs[k];
+        r.p = p;
+        r.wmode = wmode; r.eq = equilateral ? 1 : 0; r.cta = k;
+        r.counter = counter.p + k;
+        GrUnits &un = k ? d.ub : d.ua;
+        // the limb planes leave the weighted warp kernel room for 128 staged entries at two CTAs per SM
+        // (dense rows of 64 KB and more do not fit the warp kernel's 16-bit table: everything goes to the CTA kernel)
+        const bool wide = g->dn.max_rowlen >= 65535;
+        const int short_cap = wide ? 1 : (wmode == 1) ? 125 : SHORT_CAP, short_stage = (wmode == 1) ? 128 : SHORT_STAGE;
+        if (k == 0) {
+            r.p.len_lo = 2; r.p.len_hi = short_cap;
+            r.p.row_cap = std::max(16, std::min(short_stage, (g->max_row + 15) & ~15));
+            r.smem = hist_bytes + (size_t)G3_WARPS * (tables + (size_t)r.p.row_cap * (16 + (wmode ? 8 : 0)));
+            gr_dense_units(g, un, 32, r.p.len_lo, r.p.len_hi);
+            // per warp: eight warps share the CTA's histograms
+            r.p.flush = std::min<unsigned long long>(cflush, 1ull << 28);
+            r.p.wflush = std::min<unsigned long long>(gr_flush_budget(LIMB_CTA_ADDS) / G3_WARPS, LIMB_CTA_ADDS / G3_WARPS);
+        } else {
+            r.p.len_lo = short_cap + 1; r.p.len_hi = INT_MAX;
+            r.smem = hist_bytes + tables_cta + (size_t)p.row_cap * (4 + (wmode ? 8 : 0)) + 64;
+            gr_dense_units(g, un, 1, r.p.len_lo, r.p.len_hi);
+            r.p.flush = cflush;
+            r.p.wflush = std::min<unsigned long long>(gr_flush_budget(LIMB_CTA_ADDS), LIMB_CTA_ADDS);
+        }
+        r.p.n_units = un.n;
+        r.grid = 0;
+        if (un.n == 0) continue;
+        if (r.smem > g->smem_optin)
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf (gather): histogram or longest row (%d entries) does not fit in shared memory", g->max_row);
+        r.fn = gather_fn(wmode, r.eq, k, g->ooc);
+        int occ = gr_kernel_occupancy((const void *)r.fn, G3_THREADS, r.smem);
+        occ = std::max(1, std::min(occ, 8));
+        r.grid = g->sm_count * occ;
+        r.tb.cell_start = g->cell_start.p; r.tb.cell_of = g->cell_of.p; r.tb.fwd_cell = d.fwd_cell.p; r.tb.fwd_off = d.fwd_off.p;
+        r.tb.nf = d.nf.p; r.tb.rowlen = d.rowlen.p; r.tb.dbase = d.dbase.p; r.tb.units = un.units.p;
+    }
+    if (getenv("GRAMSCI_DEBUG"))
+        fprintf(stderr, "[gramsci] 3pcf gather: wmode=%d eq=%d warp: units=%d smem=%zu grid=%d | cta: units=%d smem=%zu grid=%d | row=%d dense=%.3f GB (%.2f ms)\n",
+                wmode, equilateral, runs[0].p.n_units, runs[0].smem, runs[0].grid, runs[1].p.n_units, runs[1].smem, runs[1].grid,
+                g->max_row, d.total * 1e-9, d.t_build_ms);
+
     DevBuf<unsigned long long> raw_cnt;
     DevBuf<double> raw_w;
-    counter.alloc(1);
     raw_cnt.alloc((size_t)nh);
     GR_CUDA(cudaMemsetAsync(raw_cnt.p, 0, sizeof(unsigned long long) * nh, st));
-    const int n_slots = (int)std::max<int64_t>(1, std::min<int64_t>(r.grid, ((int64_t)256 << 20) / ((int64_t)nh * 8)));
-    r.p.n_slabs = n_slots;
+    const int max_grid = std::max(1, std::max(runs[0].grid, runs[1].grid));
+    const int n_slots = (int)std::max<int64_t>(1, std::min<int64_t>(max_grid, ((int64_t)256 << 20) / ((int64_t)nh * 8)));
     if (W) {
         raw_w.alloc((size_t)nh * n_slots);
         GR_CUDA(cudaMemsetAsync(raw_w.p, 0, sizeof(double) * (size_t)nh * n_slots, st));
     }
-    r.counter = counter.p; r.raw_cnt = raw_cnt.p; r.raw_w = raw_w.p;
+    for (int k = 0; k < 2; ++k) { runs[k].p.n_slabs = n_slots; runs[k].raw_cnt = raw_cnt.p; runs[k].raw_w = raw_w.p; }
     {
         GrTimer en(st);
-        gr_for_each_tile(g, false, false, tile_3pcf_gather, &r);
+        gr_for_each_tile(g, false, false, tile_3pcf_gather, runs);
         g->t_enum_ms = en.stop();
     }
     if (equilateral) {
