@@ -150,6 +150,25 @@ __global__ void k_units(int64_t ncell, const int32_t *__restrict__ cell_start, c
     if (!pass) unit_cnt[c] = nu;
 }
 
+// (hub, spoke tile) units of the CTA gather kernel: units(c) = #tiles(c) x #listed hubs(c), where the tiles of cell c cut
+// the dense rows of every forward cell into runs of at most tile_bytes (the same arithmetic as the kernel's walk)
+__global__ void k_tile_units(int64_t ncell, const int32_t *__restrict__ cell_start, const int32_t *__restrict__ fwd_cell,
+                             const int32_t *__restrict__ nf, const int32_t *__restrict__ rowlen,
+                             const int32_t *__restrict__ ucell_off, long long tile_bytes, int64_t *__restrict__ units)
+{
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    const int nl = ucell_off[c + 1] - ucell_off[c];
+    long long nt = tile_bytes ? 0 : 1;                 // tile_bytes 0: one unit per listed hub
+    if (nl > 0 && tile_bytes)
+        for (int o = 0; o < nf[c]; ++o) {
+            const int fc = fwd_cell[c * GR_STENCIL + o];
+            const long long bytes = (long long)(cell_start[fc + 1] - cell_start[fc]) * rowlen[fc];
+            nt += max(1ll, (bytes + tile_bytes - 1) / tile_bytes);
+        }
+    units[c] = nt * nl;
+}
+
 inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64_t>(1, (n + per - 1) / per); }
 
 }  // namespace
@@ -252,6 +271,9 @@ void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int 
     GR_CUDA(cudaMemcpyAsync(&nu, off.p + nc, 4, cudaMemcpyDeviceToHost, st));
     GR_CUDA(cudaStreamSynchronize(st));
     u.units.alloc((size_t)nu + 1);
+    u.cell_off.alloc((size_t)nc + 1);
+    GR_CUDA(cudaMemcpyAsync(u.cell_off.p, off.p, sizeof(int32_t) * (nc + 1), cudaMemcpyDeviceToDevice, st));
+    u.tiles_valid = 0;
     if (nu > 0)
         k_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, g->ptr.p, max_hubs, len_lo, len_hi, 1, off.p, nullptr, u.units.p);
     GR_CUDA(cudaGetLastError());
@@ -261,4 +283,27 @@ void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int 
     u.len_lo = len_lo;
     u.len_hi = len_hi;
     g->n_launches += 5;
+}
+
+// tile-major (hub, spoke tile) unit bases of a unit list (one hub per unit), for spoke tiles of tile_bytes
+void gr_dense_tile_units(gramsci_graph *g, GrUnits &u, long long tile_bytes)
+{
+    if (u.tile_bytes == tile_bytes && u.tbase.p && u.tiles_valid) return;
+    u.tiles_valid = 1;
+    cudaStream_t st = g->stream;
+    const int64_t nc = g->ncell;
+    GrDense &d = g->dn;
+    DevBuf<int64_t> per;
+    per.alloc((size_t)nc);
+    u.tbase.alloc((size_t)nc + 1);
+    k_tile_units<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->cell_start.p, d.fwd_cell.p, d.nf.p, d.rowlen.p, u.cell_off.p,
+                                                      tile_bytes, per.p);
+    GR_CUDA(cudaGetLastError());
+    gr_exclusive_scan<int64_t, int64_t>(per.p, nc, u.tbase.p, st);
+    int64_t tot = 0;
+    GR_CUDA(cudaMemcpyAsync(&tot, u.tbase.p + nc, 8, cudaMemcpyDeviceToHost, st));
+    GR_CUDA(cudaStreamSynchronize(st));
+    u.n_tile_units = tot;
+    u.tile_bytes = tile_bytes;
+    g->n_launches += 4;
 }

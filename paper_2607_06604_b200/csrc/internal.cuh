@@ -95,6 +95,10 @@ struct GrWindow {
 #define GR_STENCIL 27
 struct GrUnits {                           // hub label ranges [x, y) inside one cell
     DevBuf<int2> units;
+    DevBuf<int32_t> cell_off;              // [ncell+1] units of cell c are units[cell_off[c] .. cell_off[c+1])
+    DevBuf<int64_t> tbase;                 // [ncell+1] CTA kernel: first (hub, spoke tile) unit of cell c
+    long long tile_bytes = 0, n_tile_units = 0;
+    int tiles_valid = 0;
     int n = 0, max_hubs = 0, len_lo = 0, len_hi = 0;
 };
 struct GrDense {
@@ -216,6 +220,7 @@ bool gr_dense_prepare(gramsci_graph *g);
 void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int32_t *idx, const uint8_t *bin, int64_t e0,
                      uint8_t *out, int64_t d0, int64_t out_bytes, cudaStream_t st);
 void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int len_hi);
+void gr_dense_tile_units(gramsci_graph *g, GrUnits &u, long long tile_bytes);
 int64_t gr_dense_rowaddr_host(gramsci_graph *g, int32_t row);      // byte offset of a row (reads the device tables)
 // query3g.cu: the gather 3pCF kernel as a tile function
 bool gr_gather_applicable(gramsci_graph *g, bool weighted, size_t hist_bytes, const char **why);

@@ -53,6 +53,10 @@ struct G3Params {
     int want_counts;
     int n_slabs;            // fp64 slabs in g_w
     int n_units;
+    long long n_tile_units;  // CTA kernel: (hub, spoke tile) units
+    long long tile_bytes;    // CTA kernel: dense bytes of one spoke tile (the rows a wave of CTAs shares in L2);
+                             // 0 = no tiling, a unit is a whole hub
+    int ncell;
     int len_lo, len_hi;     // rows this launch takes
     unsigned long long flush;    // counts: drain before the wedge budget (per warp / per CTA) passes this
     unsigned long long wflush;   // limbs: the same
@@ -63,6 +67,8 @@ struct G3Tables {
     const int32_t *cell_start, *cell_of, *fwd_cell, *fwd_off, *nf, *rowlen;
     const int64_t *dbase;
     const int2 *units;
+    const int32_t *ucell_off;   // CTA kernel: units of cell c are units[ucell_off[c] .. ucell_off[c+1])
+    const long long *tbase;     // CTA kernel: first (hub, tile) unit of cell c
 };
 
 // ---- shared memory through 32-bit shared addresses (no generic-address arithmetic in the inner loops) ----------
@@ -192,7 +198,7 @@ __device__ __forceinline__ void limbs_of(double pw, unsigned &l0, unsigned &l1, 
 // OOC: spokes whose dense row is not resident are skipped (out-of-core tiles).
 template <int WMODE, bool EQ, bool OOC>
 __global__ void __launch_bounds__(G3_THREADS)
-k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit_counter,
+k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__restrict__ unit_counter,
                    unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -246,7 +252,7 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__
     int cur_cell = -1;
     for (;;) {
         int u = 0;
-        if (lane == 0) u = (int)atomicAdd(unit_counter, 1u);
+        if (lane == 0) u = (int)atomicAdd(unit_counter, 1ull);
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= p.n_units) break;
         const int2 un = tb.units[u];
@@ -392,7 +398,7 @@ __device__ __forceinline__ void build_T_row32(const G3Tables &tb, int cj, int fc
 
 template <int WMODE, bool EQ, bool OOC>
 __global__ void __launch_bounds__(G3_THREADS)
-k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ unit_counter,
+k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restrict__ unit_counter,
                   unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -409,6 +415,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ 
     int64_t *f_dbase = (int64_t *)(f_rowlen + 32);
     double *aw = (double *)(f_dbase + 32);
     uint32_t *kx = (uint32_t *)(aw + (WMODE ? p.row_cap : 0));
+    __shared__ int f_occ[32];
     const unsigned a_hist = s_addr(hist), a_T = s_addr(T), a_kx = s_addr(kx), a_aw = s_addr(aw);
     const unsigned plane_b = (unsigned)p.nhp * 4;
     __shared__ int s_unit;
@@ -434,52 +441,108 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ 
         }
     };
 
+    // Units are (hub, spoke tile) pairs in TILE-MAJOR order inside a cell: all long hubs of cell c against the spokes
+    // in tile 0 (a run of <= tile_bytes of dense rows of one forward cell), then against tile 1, ...  The CTAs of a
+    // wave therefore gather from the same few tens of MB of dense rows, which stay in L2 (P:153-161 cuts the edge
+    // arrays into windows for the same reason one level up the hierarchy).
+    __shared__ long long s_u;
+    __shared__ int s_cell;
     int cur_cell = -1;
+    long long cur_lo = 0, cur_hi = 0;
+    int nlong = 1, nfc = 0, ubeg = 0;
     unsigned long long cb = 0, wb = 0;            // CTA-uniform: wedges since the last drain
     for (;;) {
         __syncthreads();                          // the previous unit is done: tables and staged row may be rewritten
-        if (threadIdx.x == 0) s_unit = (int)atomicAdd(unit_counter, 1u);
+        if (threadIdx.x == 0) {
+            const long long u0 = (long long)atomicAdd(unit_counter, 1ull);
+            s_u = u0;
+            if (u0 < p.n_tile_units && (u0 < cur_lo || u0 >= cur_hi)) {      // another cell: last c with tbase[c] <= u
+                int lo = 0, hi = p.ncell;
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (tb.tbase[mid] <= u0) lo = mid; else hi = mid;
+                }
+                s_cell = lo;
+            }
+        }
         __syncthreads();
-        const int u = s_unit;
-        if (u >= p.n_units) break;
-        const int2 un = tb.units[u];
-        if (un.y <= v.h_lo || un.x >= v.h_hi) continue;
-        const int c = tb.cell_of[un.x];
-        if (c != cur_cell) {
-            const int nfc = tb.nf[c];
+        const long long u = s_u;
+        if (u >= p.n_tile_units) break;
+        if (u < cur_lo || u >= cur_hi) {
+            const int c = s_cell;
+            nfc = tb.nf[c];
             const int fc = load_fwd(tb, c, nfc, lane, f_start, f_rowlen, f_dbase);      // every warp writes the same values
             for (int oj = warp; oj < nfc; oj += G3_WARPS) build_T_row32(tb, __shfl_sync(0xffffffffu, fc, oj), fc, lane, T + oj * 32);
+            // occupancy of the forward cells (tile sizes)
+            if (warp == 0) f_occ[lane] = (lane < nfc) ? tb.cell_start[fc + 1] - tb.cell_start[fc] : 0;
             cur_cell = c;
+            cur_lo = tb.tbase[c];
+            cur_hi = tb.tbase[c + 1];
+            ubeg = tb.ucell_off[c];
+            nlong = tb.ucell_off[c + 1] - ubeg;
             __syncthreads();
         }
-        for (int i = un.x; i < un.y; ++i) {
+        // (tile, hub) of this unit; tile -> (forward ordinal o, label range of its spokes)
+        const long long local = u - cur_lo;
+        int tau = (int)(local / nlong);
+        const int i = tb.units[ubeg + (int)(local % nlong)].x;
+        int o = 0, l_lo = 0, l_hi = INT_MAX;
+        if (p.tile_bytes) for (; o < nfc; ++o) {
+            const int occ_o = f_occ[o];
+            const long long bytes = (long long)occ_o * f_rowlen[o];
+            const int ns = (int)max(1ll, (bytes + p.tile_bytes - 1) / p.tile_bytes);
+            if (tau < ns) {
+                const int per = (occ_o + ns - 1) / ns;
+                l_lo = f_start[o] + tau * per;
+                l_hi = min(f_start[o] + occ_o, l_lo + per);
+                break;
+            }
+            tau -= ns;
+        }
+        {
             const bool mine = (i >= v.h_lo && i < v.h_hi) && GR_HUB_SELECTED(v, i);
             const int64_t rb = mine ? v.ptr[i] : 0, re = mine ? v.ptr[i + 1] : 0;
             const int n = (int)(re - rb);
-            if (n < p.len_lo || n > p.len_hi) continue;
-            const unsigned long long wedges = (unsigned long long)n * (n - 1) / 2;
-            __syncthreads();                      // the previous hub's entries are no longer read
+            if (n < p.len_lo || n > p.len_hi || o >= nfc || l_hi <= l_lo) continue;
+            if (OOC) { l_lo = max(l_lo, v.c_lo); l_hi = min(l_hi, v.c_hi); if (l_hi <= l_lo) continue; }
+            const int32_t *gi = v.idx_h + (rb - v.e0_h);
+            const uint8_t *gb = v.bin_h + (rb - v.e0_h);
+            // spokes of this tile = row entries with label in [l_lo, l_hi): two cooperative 256-ary search rounds
+            int a_lo = 0, a_hi = n;
+            if (p.tile_bytes) {
+                const int step = (n + G3_THREADS - 1) / G3_THREADS;
+                const int seg = (int)threadIdx.x * step;
+                int32_t last = INT_MAX;
+                if (seg < n) last = gi[min(n, seg + step) - 1];
+                const int c1 = __syncthreads_count(last < l_lo), c2 = __syncthreads_count(last < l_hi);
+                int32_t e1 = INT_MAX, e2 = INT_MAX;
+                if ((int)threadIdx.x < step && c1 * step + (int)threadIdx.x < n) e1 = gi[c1 * step + threadIdx.x];
+                if ((int)threadIdx.x < step && c2 * step + (int)threadIdx.x < n) e2 = gi[c2 * step + threadIdx.x];
+                a_lo = min(n, c1 * step + __syncthreads_count(e1 < l_lo));
+                a_hi = min(n, c2 * step + __syncthreads_count(e2 < l_hi));
+            }
+            a_hi = min(a_hi, n - 1);
+            if (a_lo >= a_hi) continue;
+            const unsigned long long wedges = (unsigned long long)(a_hi - a_lo) * (unsigned long long)(n - a_lo);
             if (cb + wedges > p.flush || (WMODE == 1 && wb + wedges > p.wflush)) {
                 drain();
                 cb = wb = 0;
             }
             cb += wedges;
             wb += wedges;
-            const int32_t *gi = v.idx_h + (rb - v.e0_h);
-            const uint8_t *gb = v.bin_h + (rb - v.e0_h);
-            for (int t = threadIdx.x; t < n; t += G3_THREADS) {
+            for (int t = a_lo + threadIdx.x; t < n; t += G3_THREADS) {
                 const int32_t k = gi[t];
-                int o = 0;
+                int ok = 0;
 #pragma unroll
                 for (int step = 16; step > 0; step >>= 1)
-                    if (f_start[o + step] <= k) o += step;
-                kx[t] = (unsigned)(k - f_start[o]) | ((unsigned)o << 16) | ((unsigned)gb[t] << 21);
+                    if (f_start[ok + step] <= k) ok += step;
+                kx[t] = (unsigned)(k - f_start[ok]) | ((unsigned)ok << 16) | ((unsigned)gb[t] << 21);
                 if (WMODE) aw[t] = v.w[k];
             }
             __syncthreads();
             const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
             unsigned long long hbud = 0;          // WMODE 1: wedges of this hub since the last drain (rows beyond 724 entries)
-            for (int a0 = 0; a0 < n - 1; a0 += G3_WARPS) {
+            for (int a0 = a_lo; a0 < a_hi; a0 += G3_WARPS) {
                 if (WMODE == 1 && wedges > p.wflush) {
                     hbud += (unsigned long long)G3_WARPS * (unsigned long long)(n - a0);
                     if (hbud > p.wflush) {
@@ -490,21 +553,17 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ 
                     }
                 }
                 const int a = a0 + warp;
-                if (a >= n - 1) continue;
+                if (a >= a_hi) continue;
                 // ---- the spoke (warp-uniform) ----
                 const unsigned ea = lds_u32(a_kx + 4u * a);
                 const int oj = (ea >> 16) & 31, pj = ea & 0xffffu;
                 const unsigned ba = ea >> 21;
-                if (OOC) {
-                    const int32_t j = f_start[oj] + pj;
-                    if (j < v.c_lo || j >= v.c_hi) continue;            // its dense row is not resident
-                }
                 const uint8_t *row = v.dense + (f_dbase[oj] + (int64_t)pj * f_rowlen[oj] - v.d0);
                 const unsigned a_Tj = a_T + (unsigned)oj * 128u;
                 const unsigned a_hj = EQ ? a_hist + ba * 4u : a_hist + ba * nb24;
                 const double wia = WMODE ? wi * lds_f64(a_aw + 8u * a) : 0.0;
-                constexpr int U = 4;
-                for (int t0 = a + 1; t0 < n; t0 += 32 * U) {
+                auto chunk = [&](int t0, auto Uc) {
+                    constexpr int U = decltype(Uc)::value;
                     unsigned kk[U], off[U], bv[U];
                     double wk[U];
 #pragma unroll
@@ -534,7 +593,10 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ 
                             if (EQ ? (bv[q] == ba) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], wia * wk[q]);
                         }
                     }
-                }
+                };
+                int t0 = a + 1;
+                for (; t0 + 128 <= n; t0 += 128) chunk(t0, std::integral_constant<int, 4>());
+                for (; t0 < n; t0 += 32) chunk(t0, std::integral_constant<int, 1>());
             }
         }
     }
@@ -542,12 +604,12 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned int *__restrict__ 
     drain();
 }
 
-typedef void (*gather_kernel_t)(GrView, G3Params, G3Tables, unsigned int *, unsigned long long *, double *);
+typedef void (*gather_kernel_t)(GrView, G3Params, G3Tables, unsigned long long *, unsigned long long *, double *);
 
 struct G3Run {
     G3Params p;
     G3Tables tb;
-    unsigned int *counter;
+    unsigned long long *counter;
     unsigned long long *raw_cnt;
     double *raw_w;
     int grid, wmode, eq, cta;
@@ -575,7 +637,7 @@ void tile_3pcf_gather(gramsci_graph *g, const GrView &v, void *user, cudaStream_
     for (int k = 0; k < 2; ++k) {
         G3Run *r = &runs[k];
         if (r->p.n_units == 0) continue;
-        GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned int), st));
+        GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned long long), st));
         r->fn<<<r->grid, G3_THREADS, r->smem, st>>>(v, r->p, r->tb, r->counter, r->raw_cnt, r->raw_w);
         GR_CUDA(cudaGetLastError());
         g->n_launches += 1;
@@ -649,7 +711,7 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
 
     G3Run runs[2];
     GrDense &d = g->dn;
-    DevBuf<unsigned int> counter;
+    DevBuf<unsigned long long> counter;
     counter.alloc(2);
     const unsigned long long cflush = gr_flush_budget(0xE0000000ull);
     for (int k = 0; k < 2; ++k) {
@@ -674,6 +736,15 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
             r.p.len_lo = short_cap + 1; r.p.len_hi = INT_MAX;
             r.smem = hist_bytes + tables_cta + (size_t)p.row_cap * (4 + (wmode ? 8 : 0)) + 64;
             gr_dense_units(g, un, 1, r.p.len_lo, r.p.len_hi);
+            long long tile_mb = 64;
+            if (const char *e = getenv("GRAMSCI_TILE_MB")) tile_mb = std::max(1ll, atoll(e));
+            // spoke tiles pay when a hub's spokes (thousands of dense rows of tens of KB) overflow L2 between two hubs
+            const bool tiled = g->n_edges / std::max<int64_t>(g->n, 1) >= 512 || getenv("GRAMSCI_TILE_MB");
+            if (!tiled) tile_mb = 0;
+            if (un.n > 0) gr_dense_tile_units(g, un, tile_mb << 20);
+            r.p.tile_bytes = tile_mb << 20;
+            r.p.n_tile_units = un.n > 0 ? un.n_tile_units : 0;
+            r.p.ncell = (int)g->ncell;
             r.p.flush = cflush;
             r.p.wflush = std::min<unsigned long long>(gr_flush_budget(LIMB_CTA_ADDS), LIMB_CTA_ADDS);
         }
@@ -688,6 +759,7 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
         r.grid = g->sm_count * occ;
         r.tb.cell_start = g->cell_start.p; r.tb.cell_of = g->cell_of.p; r.tb.fwd_cell = d.fwd_cell.p; r.tb.fwd_off = d.fwd_off.p;
         r.tb.nf = d.nf.p; r.tb.rowlen = d.rowlen.p; r.tb.dbase = d.dbase.p; r.tb.units = un.units.p;
+        r.tb.ucell_off = un.cell_off.p; r.tb.tbase = (const long long *)un.tbase.p;
     }
     if (getenv("GRAMSCI_DEBUG"))
         fprintf(stderr, "[gramsci] 3pcf gather: wmode=%d eq=%d warp: units=%d smem=%zu grid=%d | cta: units=%d smem=%zu grid=%d | row=%d dense=%.3f GB (%.2f ms)\n",
