@@ -782,9 +782,12 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     g->ooc = 0;
     if (g->cap_bytes && ((uint64_t)E * bpe > g->cap_bytes || n_windows_forced > 1)) {
         g->ooc = 1;
-        // four window buffers must fit under the cap (hub + search, double buffered)
+        // four window buffers must fit under the cap (hub + search, double buffered); on a spatially relabelled
+        // graph a window buffer also holds the dense cell-block rows expanded from its CSR rows (gather kernel)
+        uint64_t total = (uint64_t)E * bpe;
+        if (g->spatial && gr_dense_tables(g)) total += (uint64_t)g->dn.total;
         uint64_t per = g->cap_bytes / 4;
-        W = (int)(((uint64_t)E * bpe + per - 1) / std::max<uint64_t>(per, 1));
+        W = (int)((total + per - 1) / std::max<uint64_t>(per, 1));
         W = std::max(W, 2);
     }
     if (n_windows_forced > 0) { W = n_windows_forced; g->ooc = (g->cap_bytes != 0); }
@@ -817,6 +820,15 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             g->windows.push_back(w);
             r = r2;
         }
+    }
+
+    if (g->ooc && g->spatial && gr_dense_tables(g)) {      // dense byte range of every window
+        std::vector<int32_t> rows;
+        for (auto &w : g->windows) rows.push_back(w.row_lo);
+        rows.push_back((int32_t)n);
+        std::vector<int64_t> addr(rows.size());
+        gr_dense_rowaddrs(g, rows.data(), (int)rows.size(), addr.data());
+        for (size_t k = 0; k < g->windows.size(); ++k) { g->windows[k].d_lo = addr[k]; g->windows[k].d_hi = addr[k + 1]; }
     }
 
     DevBuf<int32_t> stats;

@@ -174,7 +174,7 @@ inline unsigned blocks_for(int64_t n, int per) { return (unsigned)std::max<int64
 }  // namespace
 
 // Layout tables (any spatial graph); false + reason when the structure does not apply.
-static bool dense_tables(gramsci_graph *g)
+bool gr_dense_tables(gramsci_graph *g)
 {
     GrDense &d = g->dn;
     if (d.state != 0) return d.state > 0;
@@ -209,19 +209,18 @@ static bool dense_tables(gramsci_graph *g)
     return true;
 }
 
-int64_t gr_dense_rowaddr_host(gramsci_graph *g, int32_t row)
+void gr_dense_rowaddrs(gramsci_graph *g, const int32_t *h_rows, int nrows, int64_t *h_out)
 {
     GrDense &d = g->dn;
     DevBuf<int32_t> r;
     DevBuf<int64_t> a;
-    r.alloc(1);
-    a.alloc(1);
-    int64_t out = 0;
-    GR_CUDA(cudaMemcpyAsync(r.p, &row, 4, cudaMemcpyHostToDevice, g->stream));
-    k_rowaddr<<<1, 32, 0, g->stream>>>(r.p, 1, g->n, g->cell_of.p, g->cell_start.p, d.rowlen.p, d.dbase.p, d.total, a.p);
-    GR_CUDA(cudaMemcpyAsync(&out, a.p, 8, cudaMemcpyDeviceToHost, g->stream));
+    r.alloc((size_t)nrows);
+    a.alloc((size_t)nrows);
+    GR_CUDA(cudaMemcpyAsync(r.p, h_rows, 4 * (size_t)nrows, cudaMemcpyHostToDevice, g->stream));
+    k_rowaddr<<<blocks_for(nrows, 128), 128, 0, g->stream>>>(r.p, nrows, g->n, g->cell_of.p, g->cell_start.p, d.rowlen.p,
+                                                             d.dbase.p, d.total, a.p);
+    GR_CUDA(cudaMemcpyAsync(h_out, a.p, 8 * (size_t)nrows, cudaMemcpyDeviceToHost, g->stream));
     GR_CUDA(cudaStreamSynchronize(g->stream));
-    return out;
 }
 
 void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int32_t *idx, const uint8_t *bin, int64_t e0,
@@ -240,7 +239,7 @@ void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int
 bool gr_dense_prepare(gramsci_graph *g)
 {
     GrDense &d = g->dn;
-    if (!dense_tables(g)) return false;
+    if (!gr_dense_tables(g)) return false;
     if (g->ooc || d.bytes.p) return true;
     GrTimer t(g->stream);
     size_t fr = 0, tot = 0;

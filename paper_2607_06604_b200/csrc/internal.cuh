@@ -81,6 +81,7 @@ struct DevBuf {
 struct GrWindow {
     int32_t row_lo = 0, row_hi = 0;   // rows [row_lo,row_hi)
     int64_t e_lo = 0, e_hi = 0;       // edges [e_lo,e_hi), e_lo rounded down to a multiple of 16
+    int64_t d_lo = 0, d_hi = 0;       // dense cell-block rows of these rows: bytes [d_lo,d_hi) (spatial graphs)
 };
 
 // hub filter of the enumeration kernels (hub_stride: sampled partial result; shard_*: one shard of a multi-GPU run)
@@ -215,13 +216,14 @@ void gr_work_counters(gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_el
 
 // dense.cu: layout tables + dense rows (in-core) for the gather kernel; returns false when not applicable
 bool gr_dense_prepare(gramsci_graph *g);
+bool gr_dense_tables(gramsci_graph *g);                 // layout tables only (what a capped build needs)
+void gr_dense_rowaddrs(gramsci_graph *g, const int32_t *h_rows, int nrows, int64_t *h_out);
 // expand the CSR rows [row_lo,row_hi) (edge arrays starting at edge e0) into dense rows at `out` (= row row_lo)
 // (`out` + rowaddr(row) - d0 is where a row lands; the first out_bytes bytes of `out` are reset to 0xFF)
 void gr_dense_expand(gramsci_graph *g, int32_t row_lo, int32_t row_hi, const int32_t *idx, const uint8_t *bin, int64_t e0,
                      uint8_t *out, int64_t d0, int64_t out_bytes, cudaStream_t st);
 void gr_dense_units(gramsci_graph *g, GrUnits &u, int max_hubs, int len_lo, int len_hi);
 void gr_dense_tile_units(gramsci_graph *g, GrUnits &u, long long tile_bytes);
-int64_t gr_dense_rowaddr_host(gramsci_graph *g, int32_t row);      // byte offset of a row (reads the device tables)
 // query3g.cu: the gather 3pCF kernel as a tile function
 bool gr_gather_applicable(gramsci_graph *g, bool weighted, size_t hist_bytes, const char **why);
 void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilateral);
@@ -234,7 +236,8 @@ void gr_exclusive_scan(const InT *d_in, int64_t n, OutT *d_out, cudaStream_t st)
 struct GrTileRunner;
 typedef void (*gr_tile_fn)(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st);
 // hub_only: visit each hub window once with no search window (2pCF sweep, work counters)
-void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user);
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense = false);
+int gr_tiler_slots(const gramsci_graph *g, bool need_pix, bool need_dense);
 
 // host helpers (canon.cpp part of api.cu)
 int gr_canon4(int nb, const int t[6], int c[6]);   // returns chirality factor

@@ -805,12 +805,13 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         const char *why = "";
         const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
         const size_t hist_bytes = planes * (size_t)((nh + 31) & ~31) * 4;
-        if (!g->ooc && gr_gather_applicable(g, d_wsum != nullptr, hist_bytes, &why)) {
+        if (gr_gather_applicable(g, d_wsum != nullptr, hist_bytes, &why)) {
             gr_3pcf_gather(g, d_counts, d_wsum, 0);
+            g->t_query_ms = total.stop();          // includes the one-off expansion of the dense rows
             return;
         }
         if (g->algo == GRAMSCI_ALGO_GATHER)
-            GR_FAIL(GRAMSCI_ERANGE, "3pcf: the gather kernel does not apply to this graph (%s)", g->ooc ? "device-memory cap" : why);
+            GR_FAIL(GRAMSCI_ERANGE, "3pcf: the gather kernel does not apply to this graph (%s)", why);
     }
 
     Q3Run r;

@@ -34,6 +34,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <type_traits>
+#include <vector>
 
 namespace {
 
@@ -53,6 +54,7 @@ struct G3Params {
     int want_counts;
     int n_slabs;            // fp64 slabs in g_w
     int n_units;
+    long long u_end;         // this launch takes units [value of the counter at launch, u_end)
     long long n_tile_units;  // CTA kernel: (hub, spoke tile) units
     long long tile_bytes;    // CTA kernel: dense bytes of one spoke tile (the rows a wave of CTAs shares in L2);
                              // 0 = no tiling, a unit is a whole hub
@@ -254,7 +256,7 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
         int u = 0;
         if (lane == 0) u = (int)atomicAdd(unit_counter, 1ull);
         u = __shfl_sync(0xffffffffu, u, 0);
-        if (u >= p.n_units) break;
+        if (u >= (int)p.u_end) break;
         const int2 un = tb.units[u];
         if (un.y <= v.h_lo || un.x >= v.h_hi) continue;
         const int c = tb.cell_of[un.x];
@@ -456,7 +458,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
         if (threadIdx.x == 0) {
             const long long u0 = (long long)atomicAdd(unit_counter, 1ull);
             s_u = u0;
-            if (u0 < p.n_tile_units && (u0 < cur_lo || u0 >= cur_hi)) {      // another cell: last c with tbase[c] <= u
+            if (u0 < p.u_end && (u0 < cur_lo || u0 >= cur_hi)) {      // another cell: last c with tbase[c] <= u
                 int lo = 0, hi = p.ncell;
                 while (hi - lo > 1) {
                     const int mid = (lo + hi) >> 1;
@@ -467,7 +469,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
         }
         __syncthreads();
         const long long u = s_u;
-        if (u >= p.n_tile_units) break;
+        if (u >= p.u_end) break;
         if (u < cur_lo || u >= cur_hi) {
             const int c = s_cell;
             nfc = tb.nf[c];
@@ -509,7 +511,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
             const uint8_t *gb = v.bin_h + (rb - v.e0_h);
             // spokes of this tile = row entries with label in [l_lo, l_hi): two cooperative 256-ary search rounds
             int a_lo = 0, a_hi = n;
-            if (p.tile_bytes) {
+            if (p.tile_bytes || OOC) {
                 const int step = (n + G3_THREADS - 1) / G3_THREADS;
                 const int seg = (int)threadIdx.x * step;
                 int32_t last = INT_MAX;
@@ -615,6 +617,7 @@ struct G3Run {
     int grid, wmode, eq, cta;
     size_t smem;
     gather_kernel_t fn;
+    std::vector<long long> h_ubeg, h_uend;      // out-of-core: unit range of every hub window
 };
 
 template <int WMODE, bool EQ>
@@ -637,8 +640,24 @@ void tile_3pcf_gather(gramsci_graph *g, const GrView &v, void *user, cudaStream_
     for (int k = 0; k < 2; ++k) {
         G3Run *r = &runs[k];
         if (r->p.n_units == 0) continue;
-        GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned long long), st));
-        r->fn<<<r->grid, G3_THREADS, r->smem, st>>>(v, r->p, r->tb, r->counter, r->raw_cnt, r->raw_w);
+        // units whose hubs can lie in this tile's hub window (units are in label order; cells are label ranges)
+        G3Params p = r->p;
+        long long u_begin = 0;
+        p.u_end = r->cta ? r->p.n_tile_units : (long long)r->p.n_units;
+        if (g->ooc && !r->h_ubeg.empty()) {
+            size_t w = 0;
+            while (w + 1 < g->windows.size() && g->windows[w].row_lo != v.h_lo) ++w;
+            u_begin = r->h_ubeg[w];
+            p.u_end = r->h_uend[w];
+        }
+        if (p.u_end <= u_begin) continue;
+        if (u_begin == 0) {
+            GR_CUDA(cudaMemsetAsync(r->counter, 0, sizeof(unsigned long long), st));
+        } else {                     // (a pageable host source is staged before the call returns)
+            const unsigned long long ub = (unsigned long long)u_begin;
+            GR_CUDA(cudaMemcpyAsync(r->counter, &ub, sizeof ub, cudaMemcpyHostToDevice, st));
+        }
+        r->fn<<<r->grid, G3_THREADS, r->smem, st>>>(v, p, r->tb, r->counter, r->raw_cnt, r->raw_w);
         GR_CUDA(cudaGetLastError());
         g->n_launches += 1;
     }
@@ -676,6 +695,10 @@ bool gr_gather_applicable(gramsci_graph *g, bool weighted, size_t hist_bytes, co
         return false;
     }
     if (!gr_dense_prepare(g)) { if (why) *why = g->dn.why; return false; }
+    if (g->ooc && gr_tiler_slots(g, false, true) < 2) {
+        if (why) *why = "device_mem_cap_bytes too small for two windows with their dense rows";
+        return false;
+    }
     return true;
 }
 
@@ -761,6 +784,37 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
         r.tb.nf = d.nf.p; r.tb.rowlen = d.rowlen.p; r.tb.dbase = d.dbase.p; r.tb.units = un.units.p;
         r.tb.ucell_off = un.cell_off.p; r.tb.tbase = (const long long *)un.tbase.p;
     }
+    if (g->ooc) {
+        // hub window -> unit range: cells of its first and last row, then the per-cell unit offsets
+        const size_t Wn = g->windows.size();
+        std::vector<int32_t> c_lo(Wn), c_hi(Wn);
+        for (size_t w = 0; w < Wn; ++w) {
+            const GrWindow &gw = g->windows[w];
+            c_lo[w] = c_hi[w] = 0;
+            if (gw.row_hi > gw.row_lo) {
+                GR_CUDA(cudaMemcpyAsync(&c_lo[w], g->cell_of.p + gw.row_lo, 4, cudaMemcpyDeviceToHost, st));
+                GR_CUDA(cudaMemcpyAsync(&c_hi[w], g->cell_of.p + gw.row_hi - 1, 4, cudaMemcpyDeviceToHost, st));
+            }
+        }
+        GR_CUDA(cudaStreamSynchronize(st));
+        for (int k = 0; k < 2; ++k) {
+            G3Run &r = runs[k];
+            if (r.p.n_units == 0) continue;
+            GrUnits &un = k ? d.ub : d.ua;
+            std::vector<int32_t> off((size_t)g->ncell + 1);
+            std::vector<int64_t> tb((size_t)g->ncell + 1);
+            GR_CUDA(cudaMemcpyAsync(off.data(), un.cell_off.p, 4 * off.size(), cudaMemcpyDeviceToHost, st));
+            if (k) GR_CUDA(cudaMemcpyAsync(tb.data(), un.tbase.p, 8 * tb.size(), cudaMemcpyDeviceToHost, st));
+            GR_CUDA(cudaStreamSynchronize(st));
+            r.h_ubeg.resize(Wn);
+            r.h_uend.resize(Wn);
+            for (size_t w = 0; w < Wn; ++w) {
+                const bool empty = g->windows[w].row_hi <= g->windows[w].row_lo;
+                r.h_ubeg[w] = empty ? 0 : (k ? tb[c_lo[w]] : off[c_lo[w]]);
+                r.h_uend[w] = empty ? 0 : (k ? tb[c_hi[w] + 1] : off[c_hi[w] + 1]);
+            }
+        }
+    }
     if (getenv("GRAMSCI_DEBUG"))
         fprintf(stderr, "[gramsci] 3pcf gather: wmode=%d eq=%d warp: units=%d smem=%zu grid=%d | cta: units=%d smem=%zu grid=%d | row=%d dense=%.3f GB (%.2f ms)\n",
                 wmode, equilateral, runs[0].p.n_units, runs[0].smem, runs[0].grid, runs[1].p.n_units, runs[1].smem, runs[1].grid,
@@ -779,7 +833,7 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
     for (int k = 0; k < 2; ++k) { runs[k].p.n_slabs = n_slots; runs[k].raw_cnt = raw_cnt.p; runs[k].raw_w = raw_w.p; }
     {
         GrTimer en(st);
-        gr_for_each_tile(g, false, false, tile_3pcf_gather, runs);
+        gr_for_each_tile(g, false, false, tile_3pcf_gather, runs, true);
         g->t_enum_ms = en.stop();
     }
     if (equilateral) {

@@ -16,6 +16,8 @@ namespace {
 struct Slot {
     DevBuf<int32_t> idx;
     DevBuf<uint8_t> bin, pix;
+    DevBuf<uint8_t> dense;         // dense cell-block rows of window `dense_wid`, expanded on the device from idx/bin
+    int dense_wid = -1;
     int wid = -1;
     cudaEvent_t ready = nullptr, done = nullptr;
     uint64_t stamp = 0;
@@ -23,7 +25,19 @@ struct Slot {
 
 }  // namespace
 
-void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user)
+// window buffers that fit under the cap (each: the window's CSR arrays, plus its dense rows when asked for)
+int gr_tiler_slots(const gramsci_graph *g, bool need_pix, bool need_dense)
+{
+    const int W = (int)g->windows.size();
+    const uint64_t bpe = 5 + ((g->has_pix && need_pix) ? 1 : 0);
+    int64_t maxlen = 0, maxdense = 0;
+    for (auto &w : g->windows) { maxlen = std::max(maxlen, w.e_hi - w.e_lo); maxdense = std::max(maxdense, w.d_hi - w.d_lo); }
+    if (!need_dense) maxdense = 0;
+    const int K = (int)std::min<uint64_t>((uint64_t)W, g->cap_bytes / std::max<uint64_t>(1, (uint64_t)maxlen * bpe + (uint64_t)maxdense));
+    return std::min(K, 8);
+}
+
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense)
 {
     cudaStream_t st = g->stream;
     GrView v;
@@ -50,10 +64,10 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
 
     const int W = (int)g->windows.size();
     const uint64_t bpe = 5 + (g->has_pix ? 1 : 0);
-    int64_t maxlen = 0;
-    for (auto &w : g->windows) maxlen = std::max(maxlen, w.e_hi - w.e_lo);
-    int K = (int)std::min<uint64_t>((uint64_t)W, g->cap_bytes / std::max<uint64_t>(1, (uint64_t)maxlen * bpe));
-    K = std::min(K, 8);
+    int64_t maxlen = 0, maxdense = 0;
+    for (auto &w : g->windows) { maxlen = std::max(maxlen, w.e_hi - w.e_lo); maxdense = std::max(maxdense, w.d_hi - w.d_lo); }
+    if (!need_dense) maxdense = 0;
+    const int K = gr_tiler_slots(g, need_pix, need_dense);
     if (K < (hub_only ? 1 : 2)) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for two windows of %lld edges", (long long)maxlen);
 
     std::vector<Slot> slots(K);
@@ -71,6 +85,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         s.idx.alloc((size_t)maxlen + 64);
         s.bin.alloc((size_t)maxlen + 64);
         if (g->has_pix && need_pix) s.pix.alloc((size_t)maxlen + 64);
+        if (need_dense) s.dense.alloc((size_t)maxdense + 64);
         GR_CUDA(cudaEventCreateWithFlags(&s.ready, cudaEventDisableTiming));
         GR_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
     }
@@ -86,9 +101,20 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     uint64_t clock = 0;
 
     // bring window `wid` into a slot (cache hit: no copy); never evicts a slot whose bit is set in `protect`
-    auto acquire = [&](int wid, unsigned protect) -> int {
+    // the dense rows of the window in slot k (search windows of the gather kernel): memset + scatter on the copy stream,
+    // after the window's CSR has arrived
+    auto expand = [&](int k) {
+        Slot &s = slots[k];
+        if (!need_dense || s.dense_wid == s.wid) return;
+        const GrWindow &w = g->windows[s.wid];
+        if (s.dense_wid >= 0) GR_CUDA(cudaStreamWaitEvent(cs, s.done, 0));
+        gr_dense_expand(g, w.row_lo, w.row_hi, s.idx.p, s.bin.p, w.e_lo, s.dense.p, w.d_lo, w.d_hi - w.d_lo, cs);
+        GR_CUDA(cudaEventRecord(s.ready, cs));
+        s.dense_wid = s.wid;
+    };
+    auto acquire = [&](int wid, unsigned protect, bool want_dense = false) -> int {
         for (int k = 0; k < K; ++k)
-            if (slots[k].wid == wid) { slots[k].stamp = ++clock; return k; }
+            if (slots[k].wid == wid) { slots[k].stamp = ++clock; if (want_dense) expand(k); return k; }
         int victim = -1;
         for (int k = 0; k < K; ++k) {
             if (protect & (1u << k)) continue;
@@ -109,6 +135,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         GR_CUDA(cudaEventRecord(s.ready, cs));
         s.wid = wid;
         s.stamp = ++clock;
+        if (want_dense) expand(victim);
         return victim;
     };
 
@@ -121,7 +148,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     const int T = (int)tiles.size();
     for (int t = 0; t < T; ++t) {
         const int a = acquire(tiles[t].first, 0);
-        const int b = acquire(tiles[t].second, 1u << a);
+        const int b = acquire(tiles[t].second, 1u << a, need_dense);
         if (a < 0 || b < 0) GR_FAIL(GRAMSCI_ENOMEM, "window cache exhausted");
         GR_CUDA(cudaStreamWaitEvent(st, slots[a].ready, 0));
         GR_CUDA(cudaStreamWaitEvent(st, slots[b].ready, 0));
@@ -130,6 +157,8 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         v.idx_c = slots[b].idx.p; v.bin_c = slots[b].bin.p; v.pix_c = slots[b].pix.p; v.e0_c = wc.e_lo;
         v.h_lo = wh.row_lo; v.h_hi = wh.row_hi;
         v.c_lo = wc.row_lo; v.c_hi = wc.row_hi;
+        v.dense = need_dense ? slots[b].dense.p : nullptr;
+        v.d0 = wc.d_lo;
         if (g->spatial) { v.s_lo = wh.row_lo; v.s_hi = wh.row_hi; }
         else { v.s_lo = 0; v.s_hi = (int32_t)g->n; }
         fn(g, v, user, st);
@@ -139,7 +168,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         if (t + 1 < T) {
             unsigned protect = (1u << a) | (1u << b);
             int s1 = acquire(tiles[t + 1].first, protect);
-            if (s1 >= 0) acquire(tiles[t + 1].second, protect | (1u << s1));
+            if (s1 >= 0) acquire(tiles[t + 1].second, protect | (1u << s1), need_dense);
         }
     }
     GR_CUDA(cudaStreamSynchronize(st));

@@ -399,6 +399,31 @@ def test_out_of_core_equals_in_core(relabel, n_windows, cap_frac):
     assert np.array_equal(c2, og.pcf2()[0])
 
 
+@pytest.mark.parametrize("n_windows", [2, 5, 9])
+def test_out_of_core_gather_kernel(n_windows, monkeypatch):
+    """The gather kernel under a device-memory cap: a window buffer holds the CSR rows and the dense cell-block rows
+    expanded from them on the device; hubs of window h against spokes of window c.  Forced
+    (GRAMSCI_ALGO_GATHER), so a fall-back to another kernel would be an error; also with the long-row (CTA) kernel and
+    its spoke tiles, and through the histogram drains."""
+    cfg = small(33, n=6000, L=40.0, weighted=True, r_max=5.0, nb=5)
+    og, g0 = build_both(cfg)
+    oc, ow = og.pcf3()
+    csr = g0.info()["csr_bytes"]
+    _, g1 = build_both(cfg, device_mem_cap_bytes=int(csr * 4.0), n_windows=n_windows, algo=gr.ALGO_GATHER)
+    assert g1.info()["n_windows"] == n_windows
+    c, w = g1.pcf3(weighted=True)
+    assert np.array_equal(c, oc)
+    assert_weighted_close(w, ow)
+    assert g1.timing(4) >= csr * 0.99
+    monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", "2500")
+    monkeypatch.setenv("GRAMSCI_TILE_MB", "1")
+    cfg2, oc2 = _bao_replica()
+    gb = gr.gramsci_build_graph(cfg2["points"], None, cfg2["box"], cfg2["r_min"], cfg2["r_max"], cfg2["nbins"],
+                                algo=gr.ALGO_GATHER, n_windows=n_windows, device_mem_cap_bytes=2 ** 31)
+    assert gb.info()["n_windows"] == n_windows
+    assert np.array_equal(gb.pcf3()[0], oc2)
+
+
 def test_out_of_core_cap_derives_windows():
     cfg = small(32, n=8000, L=40.0, r_max=5.0, nb=4)
     og, g0 = build_both(cfg)
