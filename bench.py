@@ -1,21 +1,34 @@
 #!/usr/bin/env python
-"""bench.py -- headline benchmark: 3pCF triangles/s on BASELINE.json configs[1] (1e6 Neyman-Scott
-points, fp64 weights, + an equal-size uniform random catalogue; r<30, 15 bins) on B200.
+"""bench.py -- 3pCF triangles/s and 4pCF quadruplets/s on B200 (BASELINE.json `metric`), with the roofline of
+SURVEY.md 8(d), the end-to-end leg through host buffers and the CPU oracle timed beside it.
 
-A "step" is one pass of the whole hot path over the batch: for BOTH catalogues, graph build (cell
-list, count, scan, fill) + 3pCF enumeration + fold, through the C ABI.  `value` = triangles counted
-per second with the points already resident in HBM; `e2e` = the same through the ABI with pinned HOST
-buffers (H2D of points/weights and D2H of the histograms inside the timed region).
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg5|...]
+                  [--subs cfg5,cfg5cap,cfg3,cfg4|none] [--scaling strong|weak]
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg1|...]
+HEADLINE (the line's `value`, timed for exactly K steps after W warm-ups): BASELINE.json configs[1] ("cfg2": 1e6
+weighted Neyman-Scott points + 1e6 uniform randoms, r < 30, 15 bins).  A step is one pass of the whole hot path over
+the batch: for both catalogues, graph build (cell list, count, scan, fill; S:8(a) A1-A5) + 3pCF enumeration + fold
+(A7, A10), through the C ABI.  configs[1] is the headline because the driver times K = 20 steps: a step of the largest
+configuration (configs[4], 8.4e9 edges) takes ~18 s.  configs[4] -- the workload BASELINE's target sentence is
+about -- and configs[2], configs[3] are carried as COMPLETE SUB-RECORDS in the same line (`config.sub_records`), each
+with its own value, roofline, e2e and cpu_baseline, timed with CUDA events for one step:
+  cfg5     configs[4] with the whole graph resident      cfg5cap  the same under a 24 GiB device-memory cap (tiler)
+  cfg3     configs[2]: 4pCF + the 2pCF of the same graph  cfg4     configs[3]: weighted parity-4pCF
+L2: flushed between timed steps (256 MiB write); configs[4]'s 108 GB of graph exceed the 126 MB L2 by themselves.
 
-N > 1 (torchrun): the path shards by independent catalogues -- every rank runs the same workload with a
-different seed, no data-path collective ("weak" scaling); time = max over ranks.
---impl reference: times the CPU oracle (oracle/) on the host cores on a bounded sample of the workload.
+ROOFLINE (S:8(d)).  3pCF: t_roof = max(5 E / BW_HBM, (4 sum len N+(j) + hits) / BW_L2); frac = t_roof / t of the
+dominant enumeration launch; `bound` names the term that won.  BW_HBM = MEASURED_PEAKS.json; BW_L2 and the global RED
+rate (the 4pCF bound) are MEASURED IN THIS RUN by bench_peaks.cu (built into libbench_peaks.so) -- no constants.
+`traffic` = DRAM bytes of one launch of that kernel from the committed ncu capture named in `traffic_source`.
+
+N > 1 (torchrun): by default the hubs of ONE workload are sharded over the ranks (strong scaling; every rank builds the
+graph, one all-reduce of the histogram -- S:8(e)); per-rank enumeration times and their imbalance are reported.
+--scaling weak gives every rank its own catalogues instead.  --impl reference times the CPU oracle.
 """
 from __future__ import annotations
 
 import argparse
+import ctypes
 import hashlib
 import json
 import os
@@ -31,24 +44,40 @@ sys.path.insert(0, ROOT)
 
 import catalogues as cat  # noqa: E402
 
-
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel on cfg2, from the committed
-# ncu --set full capture (profiles/r1_c_table_3pcf_full.md)
-DRAM_TRAFFIC_BYTES = {"k_3pcf_table<weighted>": 576.641024e6 + 5.040896e6,
-                      "k_3pcf_table<counts>": 301.802240e6 + 3.864832e6}
+PEAKS_SRC = os.path.join(ROOT, "bench_peaks.cu")
+PEAKS_LIB = os.path.join(ROOT, "libbench_peaks.so")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "dram_traffic.json")     # ncu dram bytes per launch, by kernel + workload
 
 
-L2_READ_GBS = 12000.0      # L2 -> SM read bandwidth, 16-byte loads over a 32-64 MB working set (same micro-benchmark)
-RED_PEAK_GOPS = 193.0      # global RED.E.ADD.(U64|F64), spread addresses, all SMs: best line of the micro-benchmark,
-                           # whose loop overhead makes it a slight under-estimate (kernels reach ~1.1 of it)
-
-
-def load_peaks():
+def load_hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
-        d = json.load(open(p))
-        return float(d["hbm_gbs"]), "measured", d
-    return 6650.0, "fallback", {}
+        return float(json.load(open(p))["hbm_gbs"]), "MEASURED_PEAKS.json (driver, copy)"
+    return 6650.0, "fallback of B200_PROFILING.md"
+
+
+def build_peaks_lib():
+    """nvcc bench_peaks.cu -> libbench_peaks.so (in-tree; __graft_entry__.build() does the same)."""
+    if os.path.exists(PEAKS_LIB) and os.path.getmtime(PEAKS_LIB) >= os.path.getmtime(PEAKS_SRC):
+        return PEAKS_LIB
+    nvcc = os.environ.get("NVCC") or ("/usr/local/cuda/bin/nvcc" if os.path.exists("/usr/local/cuda/bin/nvcc") else "nvcc")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-shared", "-Xcompiler", "-fPIC",
+                    "-o", PEAKS_LIB, PEAKS_SRC], check=True)
+    return PEAKS_LIB
+
+
+def measure_peaks():
+    """L2 read bandwidth and atomic rates on THIS GPU, in this process (a few hundred ms)."""
+    lib = ctypes.CDLL(build_peaks_lib())
+    for f in ("peaks_l2_read_gbs", "peaks_red_f64_gops", "peaks_red_u64_gops", "peaks_smem_atom_gops", "peaks_hbm_copy_gbs"):
+        getattr(lib, f).restype = ctypes.c_double
+        getattr(lib, f).argtypes = [ctypes.c_int]
+    l2 = {mb: lib.peaks_l2_read_gbs(mb) for mb in (16, 32, 64)}
+    return {"l2_read_gbs": max(l2.values()), "l2_read_gbs_by_working_set_mb": l2,
+            "red_f64_gops": lib.peaks_red_f64_gops(3375), "red_u64_gops": lib.peaks_red_u64_gops(262144),
+            "smem_atom_gops": lib.peaks_smem_atom_gops(3375), "hbm_copy_gbs_in_run": lib.peaks_hbm_copy_gbs(1024),
+            "how": "bench_peaks.cu in this run: 16-byte loads over 16/32/64 MB working sets (best); fp64 RED into per-CTA "
+                   "slabs of 3375 bins; uint64 RED into one 8^6-bin histogram; uint32 shared atomics on 3375 bins"}
 
 
 class ClockSampler(threading.Thread):
@@ -94,37 +123,45 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# ---- multi-rank reductions (exercised on gloo by tests/test_multirank_host.py) ---------------------------------
 def rank_seed_shift(rank: int) -> int:
-    """Sharding rule for N > 1: every rank runs the same workload shape on its own seeds (independent
-    catalogues, no data-path collective)."""
+    """--scaling weak: every rank runs the same workload shape on its own seeds (no data-path collective)."""
     return 1000 * rank
 
 
-def max_over_ranks(value: float, device=None) -> float:
-    """Time of a multi-rank step = the slowest rank's device time (all-reduce MAX of one scalar; works on
-    the gloo backend with CPU tensors, which is how tests/test_multirank_host.py exercises it)."""
+def _reduce(value, op, device=None):
     import torch
     import torch.distributed as dist
     t = torch.tensor([value], dtype=torch.float64, device=device)
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(t, op=getattr(dist.ReduceOp, op))
     return float(t.item())
+
+
+def max_over_ranks(value: float, device=None) -> float:
+    """Time of a multi-rank step = the slowest rank's device time."""
+    return _reduce(value, "MAX", device)
 
 
 def sum_over_ranks(value: float, device=None) -> float:
-    """Whole-job units processed = sum over ranks (all-reduce SUM of one scalar)."""
+    return _reduce(value, "SUM", device)
+
+
+def gather_over_ranks(value: float, device=None):
+    """Every rank's value (per-rank enumeration times -> imbalance)."""
     import torch
     import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1):
+        return [float(value)]
     t = torch.tensor([value], dtype=torch.float64, device=device)
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-    return float(t.item())
+    out = [torch.zeros_like(t) for _ in range(dist.get_world_size())]
+    dist.all_gather(out, t)
+    return [float(x.item()) for x in out]
 
 
 def allreduce_hist(arr, device=None):
-    """Strong-scaling mode: every rank enumerates the hubs of its shard of ONE catalogue (shard_count = world,
-    shard_index = rank); the histograms add up to the full result with one all-reduce (SUM) -- the only
-    collective a multi-GPU run of this path needs."""
+    """Strong scaling: the shard histograms add up to the full result with ONE all-reduce (SUM) -- the only collective
+    a multi-GPU run of this path needs; integer sums keep the unweighted result bit-exact."""
     import torch
     import torch.distributed as dist
     t = torch.from_numpy(np.ascontiguousarray(arr))
@@ -135,6 +172,13 @@ def allreduce_hist(arr, device=None):
     return t.cpu().numpy()
 
 
+def imbalance(times) -> float:
+    """max / mean - 1 of the per-rank enumeration times."""
+    times = [float(t) for t in times]
+    return max(times) / (sum(times) / len(times)) - 1.0 if times and sum(times) > 0 else 0.0
+
+
+# ---- workloads ----------------------------------------------------------------------------------------------
 def workload(name: str, seed_shift: int = 0):
     """List of catalogues (dicts from catalogues.py) making up one batch."""
     if name == "cfg2":
@@ -146,7 +190,7 @@ def workload(name: str, seed_shift: int = 0):
         return [cat.config1(seed=1001 + seed_shift)]
     if name == "cfg5p":       # scaled replica of configs[4] (same density, L=425)
         return [cat.config5(seed=5001 + seed_shift, n=39_062, L=425.0)]
-    if name == "cfg5":        # configs[4] in full: 2.5e6 points, 8.4e9 edges, 42 GB of CSR (use --steps 1 --warmup 0)
+    if name in ("cfg5", "cfg5cap"):   # configs[4] in full: 2.5e6 points, 8.4e9 edges, 42 GB of CSR
         return [cat.config5(seed=5001 + seed_shift)]
     if name == "cfg3":        # configs[2]: 4pCF (+ the 2pCF of the same graph for the disconnected term)
         return [cat.config3(seed=3001 + seed_shift)]
@@ -157,60 +201,280 @@ def workload(name: str, seed_shift: int = 0):
     raise SystemExit(f"unknown workload {name}")
 
 
-# ------------------------------------------------------------------------------------------------
+WORKLOAD_NOTE = {
+    "cfg2": "BASELINE configs[1]", "cfg5": "BASELINE configs[4], graph resident", "cfg5cap": "BASELINE configs[4] under "
+    "a 24 GiB device-memory cap (out-of-core tiler)", "cfg3": "BASELINE configs[2]", "cfg4": "BASELINE configs[3]",
+    "cfg1": "BASELINE configs[0]"}
+
+
+def metric_of(kind: str):
+    return {"3pcf": ("3pCF triangles/s", "triangles/s"), "4pcf": ("4pCF quadruplets/s", "quadruplets/s"),
+            "4pcf_parity": ("parity-4pCF quadruplets/s", "quadruplets/s")}[kind]
+
+
+# ---- CPU oracle legs ------------------------------------------------------------------------------------------
+def oracle_sample(name: str, cats, budget_s: float = 8.0):
+    """The CPU oracle as it stands on a BOUNDED sample of the workload: (tuples, seconds, description).  Small
+    workloads run in full; large ones on a hub sample sized from a first short probe."""
+    import oracle
+    t0 = time.perf_counter()
+    tuples = 0
+    what = []
+    for c in cats:
+        kind = c["kind"]
+        n = c["points"].shape[0]
+        if name in ("cfg5", "cfg5cap", "cfg5p") and n > 100_000:
+            # rows found on demand from the cell list (the graph is too large to hold): sampled hubs
+            g = oracle.Graph(c["points"], c["weights"], c["box"], c["r_min"], c["r_max"], c["nbins"], lists=False)
+            hubs = np.arange(0, n, n // 48)[:48]
+            t1 = time.perf_counter()
+            cnt, _ = g.pcf3_direct(hubs[:4])
+            per = (time.perf_counter() - t1) / 4
+            k = int(max(4, min(len(hubs), budget_s / max(per, 1e-3))))
+            cnt, _ = g.pcf3_direct(hubs[:k])
+            tuples += int(cnt.sum())
+            what.append(f"{c['name']}: cell list + 3pCF walk of {k} hubs, rows found on demand")
+            continue
+        g = oracle.Graph(c["points"], c["weights"], c["box"], c["r_min"], c["r_max"], c["nbins"])
+        if kind == "3pcf":
+            cnt, _ = g.pcf3()
+            what.append(f"{c['name']}: graph build + full 3pCF walk")
+        else:
+            stride = 1
+            if g.n_edges > 3e7:                       # configs[3]: every 2048th hub
+                stride = 2048
+            elif g.n_edges > 3e6:                     # configs[2]: every 16th hub
+                stride = 16
+            res = g.pcf4(parity=(kind == "4pcf_parity"), hubs=(0, n, stride))
+            cnt = res[0]
+            what.append(f"{c['name']}: graph build + {'parity-' if kind == '4pcf_parity' else ''}4pCF walk on every "
+                        f"{stride}-th hub")
+        tuples += int(cnt.sum())
+        del g
+    dt = time.perf_counter() - t0
+    return tuples, dt, "; ".join(what)
+
+
+def cpu_baseline(name: str, cats):
+    import oracle
+    tuples, dt, what = oracle_sample(name, cats)
+    unit = metric_of(cats[0]["kind"])[1]
+    return {"value": tuples / dt, "unit": unit, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"{what}: {tuples} tuples in {dt:.1f} s"}
+
+
 def run_reference(args):
-    """The CPU oracle as it stands, on the host cores, on a bounded sample of the workload."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """--impl reference: the CPU oracle as it stands, on the host cores, each step a bounded sample of the workload."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     import oracle
     cats = workload(args.workload)
-    stride = args.ref_stride
-    tri = 0
-    t_total = 0.0
-    for _ in range(args.warmup):
-        pass  # the oracle has no warm-up state; the build below is part of every step
-    per_step = []
+    per_step, tuples, what = [], 0, ""
     for _ in range(args.steps):
-        t0 = time.perf_counter()
-        tri = 0
-        for c in cats:
-            g = oracle.Graph(c["points"], c["weights"], c["box"], c["r_min"], c["r_max"], c["nbins"])
-            cnt, _ = g.pcf3(hubs=(0, g.n, stride))
-            tri += int(cnt.sum())
-            del g
-        per_step.append(time.perf_counter() - t0)
-    t_total = float(np.mean(per_step))
-    value = tri / t_total
-    sample = (f"full graph build + 3pCF walk on every {stride}-th hub of each catalogue "
-              f"({tri} triangles per step)")
-    line = {
-        "impl": "reference", "metric": "3pCF triangles/s", "value": value, "unit": "triangles/s",
-        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "note": "CPU oracle (plain C + OpenMP), not tuned"},
-        "cpu_baseline": {"value": value, "unit": "triangles/s", "cores": oracle.threads(), "kind": "oracle",
-                         "sample": sample},
-        "e2e": {"value": value, "unit": "triangles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        tuples, dt, what = oracle_sample(args.workload, cats)
+        per_step.append(dt)
+    t = float(np.mean(per_step))
+    metric, unit = metric_of(cats[0]["kind"])
+    value = tuples / t
+    print(json.dumps({
+        "impl": "reference", "metric": metric, "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "note": "CPU oracle (plain C + OpenMP), not tuned; the oracle has no warm-up state"},
+        "cpu_baseline": {"value": value, "unit": unit, "cores": oracle.threads(), "kind": "oracle",
+                         "sample": f"{what}: {tuples} tuples per step"},
+        "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+# ---- our arm ---------------------------------------------------------------------------------------------------
+class Runner:
+    """One workload on this rank's GPU: step(), timed legs and the roofline of its dominant kernel."""
+
+    def __init__(self, name, cats, args, world=1, rank=0, strong=False):
+        import torch
+        self.torch = torch
+        self.name, self.cats, self.args = name, cats, args
+        self.world, self.rank, self.strong = world, rank, strong
+        self.cap = 24.0 if name == "cfg5cap" else args.cap_gib
+        self.dev = [(torch.from_numpy(c["points"]).cuda(), None if c["weights"] is None else torch.from_numpy(c["weights"]).cuda())
+                    for c in cats]
+        self.pin = [(torch.from_numpy(c["points"]).pin_memory(), None if c["weights"] is None else torch.from_numpy(c["weights"]).pin_memory())
+                    for c in cats]
+        self.stats = {}
+
+    def step(self, host: bool, count_work: bool = False):
+        """One pass of the hot path over the batch: (tuples, step stats, per-catalogue stats)."""
+        import paper_2607_06604_b200 as gr
+        tuples = 0
+        st = {"enum_ms": 0.0, "build_ms": 0.0, "query_ms": 0.0, "launches": 0.0, "edges": 0}
+        per = []
+        digest = hashlib.sha1()
+        for c, d, p in zip(self.cats, self.dev, self.pin):
+            pts, w = (p if host else d)
+            kind = c["kind"]
+            g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=self.args.algo,
+                                       want_pixels=(kind == "4pcf_parity"), device_mem_cap_bytes=int(self.cap * 2 ** 30),
+                                       shard_count=self.world if self.strong else 0, shard_index=self.rank if self.strong else 0)
+            st["build_ms"] += g.timing(0)
+            st["launches"] += g.timing(3)
+            pc = {"name": c["name"], "weighted": w is not None, "kind": kind}
+            if kind == "3pcf":
+                cnt, ws = g.pcf3(counts=True, weighted=(w is not None), host=host)
+            elif kind == "4pcf":
+                cnt, ws = g.pcf4(counts=True, weighted=(w is not None), host=host)
+            else:
+                cnt, _, ws, _ = g.pcf4_parity(counts=True, weighted=(w is not None), host=host)
+            enum_ms, query_ms, launches = g.timing(2), g.timing(1), g.timing(3)
+            if kind == "4pcf":                 # configs[2]: "disconnected part estimated on the same graph" (Eq. 4 needs xi)
+                g.pcf2(host=host)
+                query_ms += g.timing(1)
+                launches += g.timing(3)
+            if self.strong:                    # partial histograms of the shards -> full result on every rank
+                cnt = allreduce_hist(cnt, "cuda")
+                if ws is not None:
+                    ws = allreduce_hist(ws, "cuda")
+            digest.update(np.ascontiguousarray(cnt).tobytes())
+            pc.update(enum_ms=enum_ms, n_windows=g.info()["n_windows"], staged_bytes=g.timing(4))
+            st["enum_ms"] += enum_ms
+            st["query_ms"] += query_ms
+            st["launches"] += launches
+            t = int(cnt.sum())
+            tuples += t
+            e = g.info()["n_edges"]
+            st["edges"] += e
+            pc.update(edges=e, hits=t)
+            if count_work and kind == "3pcf":
+                sp, tl = g.work_counters()
+                pc.update(spoke=sp, tail=tl)
+            per.append(pc)
+            g.free()
+        self.stats["sha1"] = digest.hexdigest()
+        return tuples, st, per
+
+    def timed(self, host: bool, steps: int, warmup: int, flush):
+        import torch.distributed as dist
+        torch = self.torch
+        for _ in range(warmup):
+            self.step(host)
+        if self.world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        total_ms, tuples, agg, per_enum = 0.0, 0, None, None
+        for _ in range(steps):
+            flush.fill_(1)                      # flush L2 between timed iterations (not timed)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            tuples, st, per = self.step(host)
+            e1.record()
+            torch.cuda.synchronize()
+            total_ms += e0.elapsed_time(e1)
+            agg = st if agg is None else {k: agg[k] + st[k] for k in st}
+            per_enum = [p["enum_ms"] for p in per] if per_enum is None else [a + p["enum_ms"] for a, p in zip(per_enum, per)]
+        if self.world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        self.last_per = per
+        return (max_over_ranks(total_ms, "cuda") / steps, tuples, {k: v / steps for k, v in agg.items()},
+                [a / steps for a in per_enum])
+
+
+def dram_traffic(kernel_key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch from the committed ncu --set full capture."""
+    try:
+        table = json.load(open(TRAFFIC_FILE))
+        ent = table.get(kernel_key)
+        if ent:
+            return float(ent["bytes"]), f"profiles/dram_traffic.json <- {ent['source']}"
+    except Exception:
+        pass
+    return None, None
+
+
+def roofline_3pcf(name, w, launch_ms, hbm, hbm_kind, peaks):
+    """t_roof = max(5 E / BW_HBM, (4 sum len N+(j) + hits) / BW_L2) over the launch time."""
+    t_hbm = 5.0 * w["edges"] / (hbm * 1e9)
+    t_l2 = (4.0 * w["spoke"] + w["hits"]) / (peaks["l2_read_gbs"] * 1e9)
+    t_roof = max(t_hbm, t_l2)
+    bound = "l2" if t_l2 >= t_hbm else "hbm"
+    alg_bytes = (4.0 * w["spoke"] + w["hits"]) if bound == "l2" else 5.0 * w["edges"]
+    peak = peaks["l2_read_gbs"] if bound == "l2" else hbm
+    achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    kern = ("weighted 3pCF" if w["weighted"] else "3pCF counts") + f" enumeration launch on {w['name']}"
+    traffic, src = dram_traffic(f"{name}:{w['name']}")
+    return {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": t_roof * 1e3 / launch_ms,
+            "traffic": traffic, "traffic_source": src, "kernel": kern, "launch_ms": launch_ms, "t_roof_ms": t_roof * 1e3,
+            "peak_kind": ("L2->SM read bandwidth measured in this run (bench_peaks.cu)" if bound == "l2" else hbm_kind),
+            "algorithmic_bytes_per_launch": alg_bytes,
+            "units_per_launch": {"spoke_row_elements": w["spoke"], "wedges": w["tail"], "hub_spoke_pairs": w["edges"],
+                                 "hits": w["hits"]},
+            "terms_ms": {"csr_once_from_hbm": t_hbm * 1e3, "spoke_rows_and_hits_from_l2": t_l2 * 1e3},
+            "secondary": {
+                "hits_per_s": w["hits"] / (launch_ms * 1e-3),
+                "smem_atomic_rate_gops_measured": peaks["smem_atom_gops"],
+                "global_red_rate_gops_measured": peaks["red_f64_gops"],
+                "note": "one shared-memory atomic per hit (counts) and, weighted, one fp64 RED per hit on clustered "
+                        "catalogues: hits/s over these measured rates is the atomic-path utilisation"}}
+
+
+def roofline_4pcf(w, launch_ms, channels, peaks):
+    """4pCF kernels: one global RED per hit and kind of output into nb^6 raw bins; the bound is the
+    global atomic rate, measured in this run."""
+    rate = w["hits"] * channels / (launch_ms * 1e-3) / 1e9
+    peak = peaks["red_u64_gops"] if channels == 1 else min(peaks["red_u64_gops"], peaks["red_f64_gops"])
+    return {"bound": "l2-atomics", "achieved": rate, "peak": peak, "unit": "Gatomic/s", "frac": rate / peak, "traffic": None,
+            "kernel": f"k_4pcf on {w['name']}", "launch_ms": launch_ms,
+            "peak_kind": "global RED rate measured in this run (bench_peaks.cu)",
+            "units_per_launch": {"hits": w["hits"], "red_per_hit": channels}}
+
+
+def record_for(name, cats, args, peaks, hbm, hbm_kind, flush, steps, warmup, e2e_steps, world=1, rank=0, strong=False,
+               with_cpu=True):
+    """Everything the contract asks of a workload: value, e2e, roofline of the dominant launch, cpu_baseline."""
+    r = Runner(name, cats, args, world, rank, strong)
+    _, _, work = r.step(False, count_work=True)          # untimed: exact work counters of this workload
+    ms, tuples, st, enum_ms = r.timed(False, steps, warmup, flush)
+    rank_enum = gather_over_ranks(st["enum_ms"], "cuda")
+    ms_e2e = None
+    if e2e_steps > 0:
+        ms_e2e, t2, _, _ = r.timed(True, e2e_steps, 1 if steps > 1 else 0, flush)
+        assert t2 == tuples
+    total = float(tuples) if (strong or world == 1) else sum_over_ranks(float(tuples), "cuda")
+    kind0 = cats[0]["kind"]
+    metric, unit = metric_of(kind0)
+    dom = max(range(len(cats)), key=lambda k: enum_ms[k])
+    w = dict(work[dom])
+    if kind0 == "3pcf":
+        roof = roofline_3pcf(name, w, enum_ms[dom], hbm, hbm_kind, peaks)
+        roof["per_launch"] = [dict(catalogue=x["name"], launch_ms=enum_ms[k],
+                                   frac=roofline_3pcf(name, dict(x), enum_ms[k], hbm, hbm_kind, peaks)["frac"])
+                              for k, x in enumerate(work)]
+    else:
+        roof = roofline_4pcf(w, enum_ms[dom], 1 if cats[dom]["weights"] is None else 2, peaks)
+    h2d = sum(c["points"].nbytes + (0 if c["weights"] is None else c["weights"].nbytes) for c in cats)
+    nh = {"3pcf": 3, "4pcf": 6, "4pcf_parity": 6}
+    d2h = sum(8 * c["nbins"] ** nh[c["kind"]] * (1 if c["weights"] is None else 2) * (2 if c["kind"] == "4pcf_parity" else 1)
+              + (8 * c["nbins"] if c["kind"] == "4pcf" else 0) for c in cats)
+    rec = {
+        "metric": metric, "value": total / (ms * 1e-3), "unit": unit, "steps": steps, "warmup": warmup, "ms_per_step": ms,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "what": WORKLOAD_NOTE.get(name, name), "catalogues": [c["name"] for c in cats],
+                   "n_points": [int(c["points"].shape[0]) for c in cats], "tuples_per_step": tuples,
+                   "counts_sha1": r.stats.get("sha1"), "cap_gib": r.cap, "n_windows": [p["n_windows"] for p in r.last_per],
+                   "staged_bytes_per_step": sum(p["staged_bytes"] for p in r.last_per),
+                   "edges_per_step": st["edges"], "hub_spoke_edges_per_s": st["edges"] / (ms * 1e-3),
+                   "build_ms": st["build_ms"], "query_ms": st["query_ms"], "enum_kernel_ms": st["enum_ms"],
+                   "enum_kernel_ms_per_catalogue": enum_ms,
+                   "query_only_tuples_per_s": tuples / (st["query_ms"] * 1e-3) if st["query_ms"] > 0 else None,
+                   "per_rank_enum_ms": rank_enum, "enum_imbalance": imbalance(rank_enum)},
+        "e2e": None if ms_e2e is None else {"value": total / (ms_e2e * 1e-3), "unit": unit, "h2d_bytes_per_step": h2d,
+                                            "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
+        "gpu_launches": int(round(st["launches"] * steps)),
+        "roofline": roof,
     }
-    print(json.dumps(line))
-
-
-def cpu_baseline(cats, budget_s: float = 20.0):
-    import oracle
-    t0 = time.perf_counter()
-    tri = 0
-    # bounded sample (~20 s on 16 cores): the build of the full graph and every hub of each catalogue
-    stride = 1
-    for c in cats:
-        g = oracle.Graph(c["points"], c["weights"], c["box"], c["r_min"], c["r_max"], c["nbins"])
-        cnt, _ = g.pcf3(hubs=(0, g.n, stride))
-        tri += int(cnt.sum())
-        del g
-    dt = time.perf_counter() - t0
-    return {"value": tri / dt, "unit": "triangles/s", "cores": oracle.threads(), "kind": "oracle",
-            "sample": f"oracle graph build + 3pCF walk on every {stride}-th hub of each catalogue: "
-                      f"{tri} triangles in {dt:.1f} s"}
+    if with_cpu and world == 1:
+        rec["cpu_baseline"] = cpu_baseline(name, cats)
+    return rec
 
 
 def run_ours(args):
@@ -227,189 +491,61 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     gr.load_library()
+    peaks = measure_peaks()
+    hbm, hbm_kind = load_hbm_peak()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")    # > 126 MB L2
 
     strong = args.scaling == "strong" and world > 1
-    cats = workload(args.workload, seed_shift=0 if strong else rank_seed_shift(rank))
-    dev = [(torch.from_numpy(c["points"]).cuda(), None if c["weights"] is None else torch.from_numpy(c["weights"]).cuda())
-           for c in cats]
-    pin = [(torch.from_numpy(c["points"]).pin_memory(), None if c["weights"] is None else torch.from_numpy(c["weights"]).pin_memory())
-           for c in cats]
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")    # > 126 MB L2
-    stats = {}
-
-    def step(host: bool, count_work: bool = False):
-        """one pass of the hot path over the batch; returns (triangles, per-step stats, per-catalogue stats)"""
-        tri = 0
-        st = {"enum_ms": 0.0, "build_ms": 0.0, "query_ms": 0.0, "launches": 0.0, "edges": 0}
-        per = []
-        digest = hashlib.sha1()
-        for c, d, p in zip(cats, dev, pin):
-            pts, w = (p if host else d)
-            kind = c["kind"]
-            g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo,
-                                       want_pixels=(kind == "4pcf_parity"),
-                                       device_mem_cap_bytes=int(args.cap_gib * 2 ** 30),
-                                       shard_count=world if strong else 0, shard_index=rank if strong else 0)
-            st["build_ms"] += g.timing(0)
-            st["launches"] += g.timing(3)
-            if kind == "3pcf":
-                cnt, ws = g.pcf3(counts=True, weighted=(w is not None), host=host)
-            elif kind == "4pcf":
-                cnt, ws = g.pcf4(counts=True, weighted=(w is not None), host=host)
-            else:
-                cnt, _, ws, _ = g.pcf4_parity(counts=True, weighted=(w is not None), host=host)
-            if strong:                     # partial histograms of the shards -> full result on every rank
-                cnt = allreduce_hist(cnt, "cuda")
-                if ws is not None:
-                    ws = allreduce_hist(ws, "cuda")
-            digest.update(np.ascontiguousarray(cnt).tobytes())
-            pc = {"name": c["name"], "enum_ms": g.timing(2), "weighted": w is not None}
-            st["enum_ms"] += g.timing(2)
-            st["query_ms"] += g.timing(1)
-            st["launches"] += g.timing(3)
-            t = int(cnt.sum())
-            tri += t
-            e = g.info()["n_edges"]
-            st["edges"] += e
-            if count_work:
-                sp, tl = g.work_counters() if kind == "3pcf" else (0, 0)
-                # algorithmic bytes of the enumeration (DESIGN.md section 6): spoke rows + hub tails (4 B per
-                # element), b_ij per hub-spoke pair, two bin bytes per hit (+ two fp64 weights when weighted)
-                pc.update(spoke=sp, tail=tl, edges=e, hits=t,
-                          bytes=4.0 * sp + 4.0 * tl + e + 2.0 * t)
-            pc["n_windows"] = g.info()["n_windows"]
-            pc["staged_bytes"] = g.timing(4)
-            per.append(pc)
-            g.free()
-        stats["sha1"] = digest.hexdigest()
-        stats["windows"] = [p_["n_windows"] for p_ in per]
-        stats["staged_bytes"] = sum(p_["staged_bytes"] for p_ in per)
-        return tri, st, per
-
-    def timed(host: bool, steps: int, warmup: int):
-        for _ in range(warmup):
-            step(host)
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-        total_ms, tri, agg, per_agg = 0.0, 0, None, None
-        for _ in range(steps):
-            flush.fill_(1)                      # flush L2 between timed iterations (not timed)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            tri, st, per = step(host)
-            e1.record()
-            torch.cuda.synchronize()
-            total_ms += e0.elapsed_time(e1)
-            agg = st if agg is None else {k: agg[k] + st[k] for k in st}
-            per_agg = [p["enum_ms"] for p in per] if per_agg is None else [a + p["enum_ms"] for a, p in zip(per_agg, per)]
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-        return (max_over_ranks(total_ms, "cuda") / steps, tri, {k: v / steps for k, v in agg.items()},
-                [a / steps for a in per_agg])
-
+    cats = workload(args.workload, seed_shift=0 if (strong or world == 1) else rank_seed_shift(rank))
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    _, _, work = step(False, count_work=True)       # untimed: exact work counters of this workload
-    ms, tri, st, enum_ms = timed(False, args.steps, args.warmup)
+    big = args.workload in ("cfg5", "cfg5cap", "cfg4")
+    rec = record_for(args.workload, cats, args, peaks, hbm, hbm_kind, flush, args.steps, args.warmup,
+                     0 if args.skip_e2e else max(1, args.steps // 2), world, rank, strong,
+                     with_cpu=not args.no_cpu_baseline)
     clocks = sampler.stop() if rank == 0 else None
-    if args.skip_e2e:
-        ms_e2e = None
-    else:
-        ms_e2e, tri2, _, _ = timed(True, max(1, args.steps // 2), 1)
-        assert tri2 == tri
-    tri_all = float(tri) if strong else sum_over_ranks(float(tri), "cuda")
 
-    # second headline of BASELINE.json's metric: 4pCF quadruplets/s on configs[2] (query only, rank 0, untimed region)
-    four = None
-    if rank == 0 and not args.no_4pcf:
-        c3 = cat.config3()
-        g = gr.gramsci_build_graph(torch.from_numpy(c3["points"]).cuda(), None, c3["box"], c3["r_min"], c3["r_max"], c3["nbins"])
-        best = None
-        for _ in range(3):
-            ec, _ = g.pcf4()
-            best = g.timing(1) if best is None else min(best, g.timing(1))
-        four = {"workload": "cfg3", "quadruplets": int(ec.sum()), "query_ms": best,
-                "quadruplets_per_s": float(ec.sum()) / (best * 1e-3)}
-        g.free()
+    subs = {}
+    if rank == 0 and world == 1 and args.subs != "none" and not big:
+        for name in [s for s in args.subs.split(",") if s]:
+            torch.cuda.synchronize()
+            gr.gramsci_release_memory()
+            # one timed step (an 18 s step does not warm up; the first step of cfg5 also pays the growth of the memory
+            # pool to 108 GB); the capped run's overhead is taken against the resident run of this same process
+            sub = record_for(name, workload(name), args, peaks, hbm, hbm_kind, flush, 1, 0 if name != "cfg3" else 3,
+                             0 if args.skip_e2e else 1, with_cpu=not args.no_cpu_baseline)
+            sub.pop("data", None)
+            subs[name] = sub
+        if "cfg5" in subs and "cfg5cap" in subs:
+            a, b = subs["cfg5"], subs["cfg5cap"]
+            b["config"]["ooc_overhead"] = {
+                "query": b["config"]["query_ms"] / a["config"]["query_ms"] - 1.0,
+                "build_plus_query": (b["config"]["build_ms"] + b["config"]["query_ms"]) / (a["config"]["build_ms"] + a["config"]["query_ms"]) - 1.0,
+                "step": b["ms_per_step"] / a["ms_per_step"] - 1.0,
+                "identical_histograms": a["config"]["counts_sha1"] == b["config"]["counts_sha1"],
+                "paper": "~20 % on 5x5 tiles, RTX 3090 Ti (P:161)"}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    peak, peak_kind, peaks = load_peaks()
-    h2d = sum(c["points"].nbytes + (0 if c["weights"] is None else c["weights"].nbytes) for c in cats)
-    d2h = sum(8 * c["nbins"] ** 3 * (1 if c["weights"] is None else 2) for c in cats)
-    # roofline of the dominant kernel = the enumeration launch with the largest share of the step
-    dom = max(range(len(cats)), key=lambda k: enum_ms[k])
-    dw = work[dom]
-    dom_s = enum_ms[dom] * 1e-3
-    achieved = dw["bytes"] / dom_s / 1e9
-    kind0 = cats[0]["kind"]
-    unit = "triangles/s" if kind0 == "3pcf" else "quadruplets/s"
-    metric = "3pCF triangles/s" if kind0 == "3pcf" else ("4pCF quadruplets/s" if kind0 == "4pcf" else "parity-4pCF quadruplets/s")
-    if kind0 == "3pcf":
-        kern = ("k_3pcf_table" if args.algo != 2 else "k_3pcf_bsearch") + ("<weighted>" if dw["weighted"] else "<counts>")
-    else:
-        kern = "k_4pcf"
-    if kind0 == "3pcf":
-        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(kern) if args.workload == "cfg2" else None,
-                "kernel": f"{kern} on {dw['name']}", "peak_kind": f"hbm copy, {peak_kind}",
-                "launch_ms": enum_ms[dom], "algorithmic_bytes_per_launch": dw["bytes"],
-                "units_per_launch": {"spoke_row_elements": dw["spoke"], "tail_elements": dw["tail"],
-                                     "hub_spoke_pairs": dw["edges"], "hits": dw["hits"]},
-                # SURVEY 8(d): t_roof = max(CSR once from HBM, spoke rows + hit bytes from L2); fraction = t_roof / t
-                "l2_roofline": {"l2_peak_gbs": L2_READ_GBS,
-                                "t_roof_ms": 1e3 * max(5.0 * dw["edges"] / (peak * 1e9),
-                                                       (4.0 * dw["spoke"] + dw["hits"]) / (L2_READ_GBS * 1e9)),
-                                "frac": max(5.0 * dw["edges"] / (peak * 1e9),
-                                            (4.0 * dw["spoke"] + dw["hits"]) / (L2_READ_GBS * 1e9)) / dom_s},
-                "per_launch": [{"catalogue": w_["name"], "launch_ms": enum_ms[k_], "achieved": w_["bytes"] / (enum_ms[k_] * 1e-3) / 1e9,
-                                "frac": w_["bytes"] / (enum_ms[k_] * 1e-3) / 1e9 / peak} for k_, w_ in enumerate(work)],
-                "note": "algorithmic bytes = 4*sum len(N+(j)) + 4*sum len(tail) + E + 2*hits (DESIGN.md "
-                        "section 6); spoke rows are re-read from L2/L1, so this is an L2->SM figure and may "
-                        "exceed the HBM peak; traffic = dram read+write of one ncu --set full launch "
-                        "(profiles/)"}
-    else:
-        # 4pCF kernels are bound by the L2 atomic rate: one RED per hit and output channel (DESIGN.md section 6);
-        # peak = RED.E.ADD.64 rate measured on this pool's B200 by csrc/ubench_atomics.cu (profiles/r1_ubench_atomics.txt)
-        # one RED per hit and kind of output (counts, weighted sums); the parity split costs no extra RED: a hit goes
-        # to the raw histogram of its sign class and the fold forms even / odd
-        ch = 1 if cats[dom]["weights"] is None else 2
-        red_rate = dw["hits"] * ch / dom_s / 1e9
-        roof = {"bound": "l2-atomics", "achieved": red_rate, "peak": RED_PEAK_GOPS, "unit": "Gatomic/s",
-                "frac": red_rate / RED_PEAK_GOPS, "traffic": None, "kernel": f"{kern} on {dw['name']}",
-                "launch_ms": enum_ms[dom], "units_per_launch": {"hits": dw["hits"], "channels": ch}}
     line = {
-        "metric": metric, "value": tri_all / (ms * 1e-3), "unit": unit,
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
-        "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic",
-        "config": {"workload": args.workload, "catalogues": [c["name"] for c in cats],
-                   "n_points": [int(c["points"].shape[0]) for c in cats], "tuples_per_step": tri,
-                   "counts_sha1": stats.get("sha1"), "cap_gib": args.cap_gib, "n_windows": stats.get("windows"),
-                   "staged_bytes_per_step": stats.get("staged_bytes"),
-                   "edges_per_step": st["edges"], "hub_spoke_edges_per_s": st["edges"] / (ms * 1e-3),
-                   "step": "graph build + enumeration (3pCF / 4pCF / parity-4pCF by workload) + fold for every "
-                   "catalogue", "l2": "flushed between timed steps (256 MiB write); the CSR of the default workload "
-                   "(>=0.3 GB per catalogue) exceeds the 126 MB L2",
-                   "algo": args.algo, "build_ms": st["build_ms"], "query_ms": st["query_ms"],
-                   "enum_kernel_ms": st["enum_ms"], "enum_kernel_ms_per_catalogue": enum_ms,
-                   "query_only_tuples_per_s": tri / (st["query_ms"] * 1e-3), "four_pcf": four},
-        "clocks": clocks,
-        "e2e": None if ms_e2e is None else {"value": tri_all / (ms_e2e * 1e-3), "unit": unit,
-                                            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                                            "ms_per_step": ms_e2e},
-        "gpu_launches": int(round(st["launches"] * args.steps)),
-        "roofline": roof,
+        "metric": rec["metric"], "value": rec["value"], "unit": rec["unit"], "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
+        "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": dict(rec["config"], algo=args.algo,
+                       step="graph build + enumeration (3pCF / 4pCF / parity-4pCF by workload) + fold for every catalogue",
+                       l2="flushed between timed steps (256 MiB write); every workload's graph also exceeds the 126 MB L2",
+                       headline_note="BASELINE.json names no configuration for its metric; configs[1] is the headline because "
+                       "the driver times K = 20 steps and a step of configs[4] takes ~18 s; configs[4] (resident and "
+                       "under a 24 GiB cap), configs[2] and configs[3] are complete sub-records below",
+                       peaks_measured_in_run=peaks, sub_records=subs),
+        "clocks": clocks, "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"], "roofline": rec["roofline"],
     }
-    if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(cats)
+    if "cpu_baseline" in rec:
+        line["cpu_baseline"] = rec["cpu_baseline"]
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -422,14 +558,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--subs", default="cfg5,cfg5cap,cfg3,cfg4",
+                    help="sub-records carried in the line at N = 1 (comma list of workloads, or 'none')")
     ap.add_argument("--algo", type=int, default=0)
-    ap.add_argument("--ref-stride", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-4pcf", action="store_true")
-    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
-                    help="N > 1: weak = every rank its own catalogues (default); strong = the hubs of ONE workload "
-                         "sharded over the ranks (every rank builds the whole graph), histograms all-reduced")
-    ap.add_argument("--skip-e2e", action="store_true", help="big workloads only: no host-buffer leg (e2e = null)")
+    ap.add_argument("--scaling", default="strong", choices=["weak", "strong"],
+                    help="N > 1: strong (default) = the hubs of ONE workload sharded over the ranks, histograms all-reduced; "
+                         "weak = every rank its own catalogues")
+    ap.add_argument("--skip-e2e", action="store_true", help="no host-buffer leg (e2e = null)")
     ap.add_argument("--cap-gib", type=float, default=0.0,
                     help="device_mem_cap_bytes in GiB (0 = whole CSR resident); forces the out-of-core tiler")
     args = ap.parse_args()

@@ -796,12 +796,8 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     g->staged_bytes = 0;
     if (!d_counts && !d_wsum) { g->t_query_ms = total.stop(); return; }
 
-    // ---- gather kernel (query3g.cu): the default for counts wherever its dense rows apply.  Weighted sums of a
-    // clustered catalogue are bound by atomics on a few hot bins either way (fixed-point limbs in
-    // shared memory 41 ms, fp64 RED of the slot-table kernel 36 ms on cfg2-D), so by default they stay with the
-    // slot-table kernel unless the catalogue's rows are short and even (max row < 4 x mean row) ----
-    const bool even_rows = g->n > 0 && (double)g->max_row < 4.0 * (double)g->n_edges / (double)g->n;
-    if ((g->algo == GRAMSCI_ALGO_DEFAULT && (!d_wsum || even_rows)) || g->algo == GRAMSCI_ALGO_GATHER) {
+    // ---- gather kernel (query3g.cu): the default wherever its dense rows apply ----
+    if (g->algo == GRAMSCI_ALGO_DEFAULT || g->algo == GRAMSCI_ALGO_GATHER) {
         const char *why = "";
         const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
         const size_t hist_bytes = planes * (size_t)((nh + 31) & ~31) * 4;

@@ -63,6 +63,7 @@ struct G3Params {
     unsigned long long flush;    // counts: drain before the wedge budget (per warp / per CTA) passes this
     unsigned long long wflush;   // limbs: the same
     double wscale, inv_wscale;
+    int hybrid;             // WMODE 1: every other spoke goes to fp64 RED instead of the limbs (two atomic paths in parallel)
 };
 
 struct G3Tables {
@@ -331,7 +332,10 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                         const unsigned hb = s[q].y >> 11;                // byte offset of b_ij in the histogram (EQ: 4 b_ij)
                         const unsigned ah = EQ ? a_hist + hb : a_hk + hb + bv[q] * 4u;
                         if (have_cnt) sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
-                        if (WMODE == 1) {
+                        if (WMODE == 1 && p.hybrid && (q & 1)) {
+                            if (EQ ? (bv[q] == (hb >> 2)) : (bv[q] != 0xffu))
+                                atomicAdd(&my_w[(ah - a_hist) >> 2], ((wi * wa[q]) * ak) * p.inv_wscale);
+                        } else if (WMODE == 1) {
                             unsigned l0, l1, l2;
                             limbs_of((wi * wa[q]) * ak, l0, l1, l2);
                             sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], hb >> 2);
@@ -587,7 +591,9 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     for (int q = 0; q < U; ++q) {
                         const unsigned ah = EQ ? a_hj : a_hj + (kk[q] >> 21) * nb4 + bv[q] * 4u;
                         if (have_cnt) sred_inc_hit<EQ>(ah, bv[q], ba);
-                        if (WMODE == 1) {
+                        if (WMODE == 1 && p.hybrid && (q & 1)) {
+                            if (EQ ? (bv[q] == ba) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], (wia * wk[q]) * p.inv_wscale);
+                        } else if (WMODE == 1) {
                             unsigned l0, l1, l2;
                             limbs_of(wia * wk[q], l0, l1, l2);
                             sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], ba);
@@ -713,14 +719,17 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
     p.nb = nb; p.nh = nh; p.nhp = (nh + 31) & ~31;
     p.want_counts = d_counts ? 1 : 0;
     p.row_cap = std::max(16, (g->max_row + 15) & ~15);
-    // weights: fixed-point limbs when the products span a factor <= 32, else fp64 RED
+    // weights: fp64 RED into per-CTA global slabs by default (measured faster than the limbs on every workload:
+    // cfg2-D 30.9 vs 40.7 ms, uniform 1e6 points 6.8 vs 11.7 ms); GRAMSCI_WMODE=1 selects the fixed-point limbs
+    // (order-independent sums) when the products span a factor <= 32
     int wmode = 0;
     p.wscale = p.inv_wscale = 1.0;
+    p.hybrid = getenv("GRAMSCI_HYBRID") ? 1 : 0;
     if (W) {
         const double hi = g->w_absmax, lo = g->w_absmin;
-        wmode = (lo > 0.0 && std::isfinite(hi) && hi / lo <= 3.1748) ? 1 : 2;
+        wmode = 2;
         if (const char *force = getenv("GRAMSCI_WMODE"))
-            if (force[0] == '2' || (force[0] == '1' && lo > 0.0 && std::isfinite(hi))) wmode = force[0] - '0';
+            if (force[0] == '1' && lo > 0.0 && std::isfinite(hi) && hi / lo <= 3.1748) wmode = 1;
         if (wmode == 1) {
             int e = 0;
             std::frexp(hi * hi * hi, &e);                  // hi^3 < 2^e
@@ -777,7 +786,10 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
         if (r.smem > g->smem_optin)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf (gather): histogram or longest row (%d entries) does not fit in shared memory", g->max_row);
         r.fn = gather_fn(wmode, r.eq, k, g->ooc);
+        if (const char *e = getenv("GRAMSCI_CARVEOUT"))      // experiment: shared-memory carve-out in percent (L1 gets the rest)
+            cudaFuncSetAttribute((const void *)r.fn, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(e));
         int occ = gr_kernel_occupancy((const void *)r.fn, G3_THREADS, r.smem);
+        if (const char *e = getenv("GRAMSCI_OCC")) occ = std::min(occ, std::max(1, atoi(e)));
         occ = std::max(1, std::min(occ, 8));
         r.grid = g->sm_count * occ;
         r.tb.cell_start = g->cell_start.p; r.tb.cell_of = g->cell_of.p; r.tb.fwd_cell = d.fwd_cell.p; r.tb.fwd_off = d.fwd_off.p;

@@ -131,6 +131,30 @@ def test_histogram_drain_path_exact(algo, monkeypatch):
     assert np.array_equal(gg.pcf3()[0], oc)
 
 
+@pytest.mark.parametrize("budget", ["", "2500"])
+def test_weighted_fixed_point_limbs(budget, monkeypatch):
+    """GRAMSCI_WMODE=1: weighted sums of the gather kernels as 13-bit fixed-point limbs in shared memory (order-
+    independent) instead of fp64 RED atomics -- same 1e-10 bar, short and long rows, capped graph."""
+    monkeypatch.setenv("GRAMSCI_WMODE", "1")
+    if budget:
+        monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", budget)
+    for cfg in (small(13, n=4000, L=40.0, weighted=True, nb=7), cat.config2_data(seed=2103, n=12_000, L=230.0, mean_parents=120.0)):
+        og, gg = build_both(cfg, algo=gr.ALGO_GATHER)
+        oc, ow = og.pcf3()
+        c, w = gg.pcf3(weighted=True)
+        assert np.array_equal(c, oc)
+        assert_weighted_close(w, ow)
+        w2 = gg.pcf3(counts=False, weighted=True)[1]       # weights only (no count plane in shared memory)
+        assert_weighted_close(w2, ow)
+    cfg = cat.config5(seed=5102, n=3_000, L=310.0)          # rows of ~1,500 entries: CTA kernel, drains inside a hub
+    w = np.random.default_rng(9).uniform(0.5, 1.5, 3000)
+    og = oracle.Graph(cfg["points"], w, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    gg = gr.gramsci_build_graph(cfg["points"], w, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], algo=gr.ALGO_GATHER)
+    c, ws = gg.pcf3(weighted=True)
+    assert gg.info()["max_row"] > 800 and np.array_equal(c, og.pcf3()[0])
+    assert_weighted_close(ws, og.pcf3()[1])
+
+
 def test_4pcf_lut_drain_path_exact(monkeypatch):
     monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", "2000")
     monkeypatch.setenv("GRAMSCI_4PCF_LUT", "1")
@@ -615,6 +639,20 @@ def test_full_size_config5_invariants_and_cap():
     c3c, _ = g2.pcf3()
     assert g2.timing(4) > 40e9                                          # the windows really were streamed
     assert np.array_equal(c3c, c3)
+    g2.free()
+    # EXACT check in the launch configuration bench.py times (spatial labels, default kernel; 2^28-hit histogram
+    # drains are reached here): the triangles whose smallest-INTERNAL-label vertex is a multiple of `stride`, against
+    # the oracle's on-demand walk over the same points given in internal order (gramsci_export_labels)
+    stride = 8192
+    gs = gr.gramsci_build_graph(pts, None, cfg["box"], cfg["r_min"], cfg["r_max"], nb, hub_stride=stride)
+    lab = gs.export_labels()
+    cs, _ = gs.pcf3()
+    gs.free()
+    od = oracle.Graph(cfg["points"][lab], None, cfg["box"], cfg["r_min"], cfg["r_max"], nb, lists=False)
+    oc, _ = od.pcf3_direct(np.arange(0, n, stride))
+    assert oc.sum() > 5e8
+    assert np.array_equal(cs, oc)
+    assert np.all(c3 >= cs)
 
 
 def test_hub_shards_add_up_to_the_full_result():

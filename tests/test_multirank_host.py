@@ -40,6 +40,9 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
     assert np.array_equal(full, np.arange(12, dtype=np.int64) * 3), full
     wfull = bench.allreduce_hist(np.full(5, 0.25 * (rank + 1)))
     assert np.allclose(wfull, 0.75)
+    # per-rank enumeration times of a strong-scaling step and their imbalance (max / mean - 1)
+    times = bench.gather_over_ranks(fake_ms)
+    assert times == [10.0, 15.0] and abs(bench.imbalance(times) - 0.2) < 1e-12
     dist.barrier()
     np.save(os.path.join(out_dir, f"r{rank}.npy"), np.array([t, u, pts[0, 0], float(len(cats))]))
     dist.destroy_process_group()
@@ -61,6 +64,21 @@ def test_single_process_reductions_are_identity():
     assert bench.max_over_ranks(3.5) == 3.5
     assert bench.sum_over_ranks(7.0) == 7.0
     assert bench.rank_seed_shift(0) == 0 and bench.rank_seed_shift(3) != bench.rank_seed_shift(2)
+    assert bench.gather_over_ranks(2.0) == [2.0] and bench.imbalance([2.0]) == 0.0
+
+
+def test_roofline_arithmetic_reproduces_by_hand():
+    """S:8(d): frac = max(5 E / BW_HBM, (4 sum len N+(j) + hits) / BW_L2) / t -- the figure of the bench line must follow
+    from the units it prints."""
+    import bench
+    w = dict(name="x", weighted=False, edges=1.0e8, spoke=1.0e10, tail=8.0e9, hits=6.0e9)
+    peaks = dict(l2_read_gbs=12000.0, smem_atom_gops=800.0, red_f64_gops=180.0, red_u64_gops=185.0)
+    r = bench.roofline_3pcf("cfg2", w, 20.0, 6500.0, "test", peaks)
+    t_l2 = (4 * 1.0e10 + 6.0e9) / 12000e9
+    assert r["bound"] == "l2" and abs(r["frac"] - t_l2 * 1e3 / 20.0) < 1e-12
+    assert abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-12
+    r4 = bench.roofline_4pcf(dict(name="y", hits=1.5e9), 10.0, 1, peaks)
+    assert r4["bound"] == "l2-atomics" and abs(r4["frac"] - (1.5e9 / 10e-3 / 1e9) / 185.0) < 1e-12
 
 
 def test_reference_arm_line_schema():
