@@ -151,6 +151,12 @@ int gramsci_2pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
 /* 3pCF (S:8(a) A7, A10): every 3-clique once; counts/wsum [nb^3] at sorted triples. */
 int gramsci_3pcf(const gramsci_graph *g, uint64_t *counts, double *wsum);
 
+/* Equilateral 3pCF (P:135, P:257 name it as one of the four query kernels; S:8(f)-3): the 3-cliques whose three
+ * edges fall in the SAME radial bin, counts/wsum [nb] indexed by that bin -- the diagonal b1 = b2 = b3 of
+ * gramsci_3pcf, but enumerated with the restriction inside the kernel: for a hub-spoke pair (i,j) only neighbours k
+ * with b_ik == b_ij are followed, and only edges (j,k) with b_jk == b_ij count. */
+int gramsci_3pcf_equilateral(const gramsci_graph *g, uint64_t *counts, double *wsum);
+
 /* 4pCF (S:8(a) A8, A10): every 4-clique once; [nb^6] at canonical 6-tuples.
  * Requires nbins <= 16, rows shorter than 65536 entries and a resident graph (no device-memory cap:
  * GRAMSCI_EINVAL otherwise). */

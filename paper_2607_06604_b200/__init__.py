@@ -25,7 +25,7 @@ ABI_SYMBOLS = [
     "gramsci_build_graph", "gramsci_graph_info", "gramsci_export_csr", "gramsci_2pcf", "gramsci_3pcf",
     "gramsci_4pcf", "gramsci_4pcf_parity", "gramsci_num_configs", "gramsci_compact", "gramsci_zeta_disc",
     "gramsci_last_timing", "gramsci_work_counters", "gramsci_free_graph", "gramsci_last_error",
-    "gramsci_export_labels", "gramsci_release_memory",
+    "gramsci_export_labels", "gramsci_release_memory", "gramsci_3pcf_equilateral",
 ]
 
 ALGO_DEFAULT, ALGO_MERGEPATH, ALGO_BSEARCH, ALGO_BITMAP = 0, 1, 2, 3
@@ -92,7 +92,8 @@ def load_library():
                                      ctypes.POINTER(ctypes.c_int32)]
     L.gramsci_export_csr.restype = ctypes.c_int
     L.gramsci_export_csr.argtypes = [vp] * 5
-    for name, nargs in (("gramsci_2pcf", 3), ("gramsci_3pcf", 3), ("gramsci_4pcf", 3), ("gramsci_4pcf_parity", 5)):
+    for name, nargs in (("gramsci_2pcf", 3), ("gramsci_3pcf", 3), ("gramsci_3pcf_equilateral", 3), ("gramsci_4pcf", 3),
+                        ("gramsci_4pcf_parity", 5)):
         f = getattr(L, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp] * nargs
@@ -223,6 +224,13 @@ class Graph:
         c = self._out(nh, "int64", host) if counts else None
         w = self._out(nh, "float64", host) if weighted else None
         _check(load_library().gramsci_3pcf(self._h, _ptr(c), _ptr(w)))
+        return self._np(c), self._np(w)
+
+    def pcf3_equilateral(self, counts: bool = True, weighted: bool = False, host: bool = False):
+        """``gramsci_3pcf_equilateral``: [nb] histograms of the triangles with all three edges in one bin."""
+        c = self._out(self.nbins, "int64", host) if counts else None
+        w = self._out(self.nbins, "float64", host) if weighted else None
+        _check(load_library().gramsci_3pcf_equilateral(self._h, _ptr(c), _ptr(w)))
         return self._np(c), self._np(w)
 
     def pcf4(self, counts: bool = True, weighted: bool = False, host: bool = False):

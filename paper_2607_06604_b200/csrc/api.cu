@@ -440,6 +440,20 @@ extern "C" int gramsci_3pcf(const gramsci_graph *cg, uint64_t *counts, double *w
     GR_API_END
 }
 
+extern "C" int gramsci_3pcf_equilateral(const gramsci_graph *cg, uint64_t *counts, double *wsum)
+{
+    GR_API_BEGIN
+    gramsci_graph *g = const_cast<gramsci_graph *>(cg);
+    if (!g) GR_FAIL(GRAMSCI_EINVAL, "3pcf_equilateral: NULL graph");
+    gr_alloc_ctx() = g->actx;
+    OutStage<uint64_t> oc; OutStage<double> ow;
+    oc.init(counts, (size_t)g->nb);
+    ow.init(wsum, (size_t)g->nb);
+    gr_3pcf(g, oc.dev, ow.dev, 1);
+    oc.finish(g->stream); ow.finish(g->stream);
+    GR_API_END
+}
+
 extern "C" int gramsci_4pcf(const gramsci_graph *cg, uint64_t *counts, double *wsum)
 {
     GR_API_BEGIN

@@ -210,7 +210,7 @@ struct GrView {
 };
 
 void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
-void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);
+void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilateral = 0);
 void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c, double *d_even_w, double *d_odd_w);
 void gr_work_counters(gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
 

@@ -33,6 +33,7 @@ struct Q3Params {
     int weighted;
     int want_counts;
     int n_slabs;        // fp64 slabs in g_w (a CTA adds to slab blockIdx % n_slabs)
+    int equi;           // equilateral restriction (S:8(f)-3): count only b_ij == b_ik == b_jk, histogram over b_ij (nh = nb)
     unsigned long long flush;   // drain the shared uint32 histogram before the CTA's hit budget passes this
 };
 
@@ -113,7 +114,8 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
                 const int32_t *T = a_idx + a + 1;
                 const int nt = n - a - 1;
                 const int32_t t_last = T[nt - 1];
-                const int hbase = (int)a_bin[a] * nb * nb;
+                const int bij = (int)a_bin[a];
+                const int hbase = bij * nb * nb;
                 const double wij = WEIGHTED ? wi * a_w[a] : 1.0;
                 int lo = 0;
                 for (int t0 = 0; t0 < nj; t0 += 32) {
@@ -121,9 +123,10 @@ k_3pcf_bsearch(GrView v, Q3Params p, unsigned int *__restrict__ hub_counter,
                     int32_t k = (t < nj) ? B[t] : INT32_MAX;
                     int pos = nt;
                     if (k <= t_last) pos = lower_bound_s(T, lo, nt, k);
-                    const bool hit = (pos < nt) && (T[pos] == k);
+                    bool hit = (pos < nt) && (T[pos] == k);
+                    if (p.equi) hit = hit && (int)Bb[t] == bij && (int)a_bin[a + 1 + pos] == bij;
                     if (hit) {
-                        const int h = hbase + (int)a_bin[a + 1 + pos] * nb + (int)Bb[t];
+                        const int h = p.equi ? bij : hbase + (int)a_bin[a + 1 + pos] * nb + (int)Bb[t];
                         if (p.want_counts) {
                             if (p.smem_hist) atomicAdd(&hist[h], 1u);
                             else atomicAdd(&g_cnt[h], 1ull);
@@ -784,11 +787,25 @@ void gr_fold3(gramsci_graph *g, int nb, const unsigned long long *raw_cnt, const
     GR_CUDA(cudaGetLastError());
 }
 
-void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
+// the equilateral histogram [nb]: raw bins are final, only the fp64 slabs are summed
+__global__ void k_sum_eq(int nb, const unsigned long long *__restrict__ cnt, const double *__restrict__ w, int n_slabs,
+                         unsigned long long *__restrict__ out_cnt, double *__restrict__ out_w)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= nb) return;
+    if (out_cnt) out_cnt[x] = cnt[x];
+    if (out_w) {
+        double s = 0.0;
+        for (int k = 0; k < n_slabs; ++k) s += w[(size_t)k * nb + x];
+        out_w[x] = s;
+    }
+}
+
+void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilateral)
 {
     cudaStream_t st = g->stream;
     const int nb = g->nb;
-    const int64_t nh64 = (int64_t)nb * nb * nb;
+    const int64_t nh64 = equilateral ? (int64_t)nb : (int64_t)nb * nb * nb;
     if (nh64 > (int64_t)1 << 26) GR_FAIL(GRAMSCI_EINVAL, "3pcf: nbins^3 too large");
     const int nh = (int)nh64;
     GrTimer total(st);
@@ -802,7 +819,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
         const size_t hist_bytes = planes * (size_t)((nh + 31) & ~31) * 4;
         if (gr_gather_applicable(g, d_wsum != nullptr, hist_bytes, &why)) {
-            gr_3pcf_gather(g, d_counts, d_wsum, 0);
+            gr_3pcf_gather(g, d_counts, d_wsum, equilateral);
             g->t_query_ms = total.stop();          // includes the one-off expansion of the dense rows
             return;
         }
@@ -812,6 +829,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
 
     Q3Run r;
     r.p.nb = nb; r.p.nh = nh;
+    r.p.equi = equilateral ? 1 : 0;
     r.p.weighted = (d_wsum != nullptr) ? 1 : 0;
     r.p.want_counts = (d_counts != nullptr) ? 1 : 0;
     r.p.row_cap = std::max(16, (g->max_row + 15) & ~15);
@@ -822,10 +840,12 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
     r.G = 8;
     // rows of hundreds of entries and more stream from DRAM (the CSR no longer lives in L2): keep 8 windows in flight
     r.long_rows = (g->n > 0 && g->n_edges / g->n >= 512) ? 1 : 0;
-    r.use_merge = (g->algo == GRAMSCI_ALGO_MERGEPATH) ? 1 : 0;
-    if (g->algo >= GRAMSCI_ALGO_BITMAP && g->algo <= GRAMSCI_ALGO_TABLE_G8 && g->max_row >= 65535)
+    r.use_merge = (g->algo == GRAMSCI_ALGO_MERGEPATH && !equilateral) ? 1 : 0;
+    if (!equilateral && g->algo >= GRAMSCI_ALGO_BITMAP && g->algo <= GRAMSCI_ALGO_TABLE_G8 && g->max_row >= 65535)
         GR_FAIL(GRAMSCI_ERANGE, "3pcf: slot table needs rows shorter than 65535 entries (longest row %d)", g->max_row);
-    if (g->algo != GRAMSCI_ALGO_BSEARCH && !r.use_merge && g->max_row >= 2 && g->max_row < 65535) {
+    // (the equilateral restriction exists in the gather kernels and, as the fallback for graphs they do not take, in
+    //  the search kernel)
+    if (!equilateral && g->algo != GRAMSCI_ALGO_BSEARCH && !r.use_merge && g->max_row >= 2 && g->max_row < 65535) {
         gr_row_stats(g);
         const size_t hist_bytes = (((size_t)nh * 4 + 15) & ~(size_t)15) + 16;
         int best_s = -1, ptl = 0, tbl = 0;
@@ -906,7 +926,12 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum)
         gr_for_each_tile(g, false, false, tile_3pcf, &r);
         g->t_enum_ms = en.stop();
     }
-    gr_fold3(g, nb, d_counts ? raw_cnt.p : nullptr, W ? raw_w.p : nullptr, n_slots, d_counts, d_wsum);
+    if (equilateral) {
+        k_sum_eq<<<(nb + 127) / 128, 128, 0, st>>>(nb, raw_cnt.p, W ? raw_w.p : nullptr, n_slots, (unsigned long long *)d_counts, d_wsum);
+        GR_CUDA(cudaGetLastError());
+    } else {
+        gr_fold3(g, nb, d_counts ? raw_cnt.p : nullptr, W ? raw_w.p : nullptr, n_slots, d_counts, d_wsum);
+    }
     g->n_launches += 1;
     GR_CUDA(cudaStreamSynchronize(st));
     g->t_query_ms = total.stop();

@@ -4,6 +4,9 @@ the histograms the CUDA library returns.  Nothing here enumerates tuples.
 * :func:`xi_periodic`      -- 2pCF of a periodic box without randoms (reading A-12, mode b)
 * :func:`zeta3_ratio`      -- zeta = NNN / RRR per configuration from a (weighted) data and a random 3pCF
 * :func:`zeta4_connected`  -- Eq. 5: zeta_conn = zeta - zeta_disc, zeta_disc from Eq. 4 (``gramsci_zeta_disc``)
+* :func:`combined_catalogue` / :func:`signed_ratio` -- the Szapudi-Szalay form: data and randoms in ONE
+  catalogue with weights summing to +1 and -1, so that the weighted k-point sum over a bin is the expansion of
+  (D - R)^k (DD - 2DR + RR, ...); the estimate is that sum over the randoms-only sum of the same graph geometry
 """
 from __future__ import annotations
 
@@ -42,3 +45,25 @@ def zeta4_connected(zeta4: np.ndarray, xi: np.ndarray) -> np.ndarray:
     the library's host helper.  Applies to the even channel only."""
     from . import gramsci_zeta_disc
     return np.asarray(zeta4, dtype=np.float64) - gramsci_zeta_disc(np.asarray(xi, dtype=np.float64))
+
+
+def combined_catalogue(data: np.ndarray, randoms: np.ndarray, w_data=None, w_rand=None):
+    """Points and signed, normalised weights of the combined catalogue: data weights sum to +1, random
+    weights to -1.  Returns (points [N_D + N_R, 3], weights [N_D + N_R], weights of the randoms alone, sum to +1)."""
+    wd = np.ones(data.shape[0]) if w_data is None else np.asarray(w_data, dtype=np.float64)
+    wr = np.ones(randoms.shape[0]) if w_rand is None else np.asarray(w_rand, dtype=np.float64)
+    wd = wd / wd.sum()
+    wr = wr / wr.sum()
+    pts = np.ascontiguousarray(np.concatenate([data, randoms], axis=0))
+    return pts, np.concatenate([wd, -wr]), wr
+
+
+def signed_ratio(n_hist: np.ndarray, r_hist: np.ndarray) -> np.ndarray:
+    """N...N / R...R per bin (P:118 for pairs; the same form for triplets and quadruplets): n_hist = weighted sums of the
+    combined signed catalogue, r_hist = weighted sums of the randoms alone (weights summing to +1).  NaN where the
+    random sum is empty."""
+    num = np.asarray(n_hist, dtype=np.float64)
+    den = np.asarray(r_hist, dtype=np.float64)
+    out = np.full(num.shape, np.nan)
+    np.divide(num, den, out=out, where=den != 0)
+    return out

@@ -246,6 +246,44 @@ def test_range_errors_on_very_long_rows():
         ga.free()
 
 
+def _diag(h, nb):
+    return np.array([h.reshape(nb, nb, nb)[b, b, b] for b in range(nb)])
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(algo=gr.ALGO_GATHER), dict(algo=gr.ALGO_BSEARCH), dict(relabel=2),
+                                  dict(relabel=2, hub_stride=3)])
+def test_3pcf_equilateral(opts):
+    """S:8(f)-3 (the equilateral 3pCF is one of the four query kernels): triangles with all three edges
+    in one radial bin, restricted inside the kernel, against the diagonal of the oracle's full 3pCF -- the gather
+    kernels (short rows, long rows), the search-kernel fallback (caller labels), weighted, and under a memory cap."""
+    stride = opts.get("hub_stride", 1)
+    cfg = cat.config1()
+    og, gg = build_both(cfg, **opts)
+    oc, _ = og.pcf3(hubs=(0, og.n, stride))
+    c, _ = gg.pcf3_equilateral()
+    assert c.shape == (cfg["nbins"],) and c.sum() > 1000
+    assert np.array_equal(c, _diag(oc, cfg["nbins"]))
+    assert np.array_equal(gg.pcf3_equilateral(host=True)[0], c)
+    # clustered replica of configs[1], weighted
+    cfg = cat.config2_data(seed=2104, n=15_625, L=250.0, mean_parents=156.25)
+    og, gg = build_both(cfg, **opts)
+    oc, ow = og.pcf3(hubs=(0, og.n, stride))
+    c, w = gg.pcf3_equilateral(weighted=True)
+    assert c.sum() > 1e5 and np.array_equal(c, _diag(oc, cfg["nbins"]))
+    assert_weighted_close(w, _diag(ow, cfg["nbins"]))
+    if stride == 1:
+        # the same graph under a device-memory cap (windows streamed from host memory)
+        csr = gg.info()["csr_bytes"]
+        _, gc = build_both(cfg, device_mem_cap_bytes=int(csr * 4), n_windows=4, **opts)
+        c2, w2 = gc.pcf3_equilateral(weighted=True)
+        assert gc.info()["n_windows"] == 4 and np.array_equal(c2, c)
+        assert_weighted_close(w2, _diag(ow, cfg["nbins"]))
+        # rows of thousands of entries, r_min > 0
+        cfg, oc = _bao_replica()
+        gb = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], **opts)
+        assert np.array_equal(gb.pcf3_equilateral()[0], _diag(oc, cfg["nbins"]))
+
+
 def test_edge_cases():
     torch = _torch()
     # empty catalogue, single point, no edges, one triangle
@@ -256,6 +294,7 @@ def test_edge_cases():
         assert c.sum() == 0
         c2, _ = g.pcf2(host=True)
         assert c2.sum() == 0
+        assert g.pcf3_equilateral(host=True)[0].sum() == 0
     tri = np.array([[1.0, 1.0, 1.0], [1.5, 1.0, 1.0], [1.0, 1.9, 1.0]])
     g = gr.gramsci_build_graph(tri, None, None, 0.0, 3.0, 3)
     og = oracle.Graph(tri, None, None, 0.0, 3.0, 3)
@@ -717,3 +756,86 @@ def test_signed_weights():
     assert np.array_equal(ec, rec) and np.array_equal(oc, roc)
     assert_weighted_close(ew, rew, scale=sc)
     assert_weighted_close(ow, row, scale=sc)
+
+
+# ---- estimator layer end to end (S:8(f)-1) ---------------------------------------------------------
+def test_signed_combined_catalogue_is_dd_minus_2dr_plus_rr():
+    """with data weights summing to +1 and random weights to -1, the weighted pair sum of the COMBINED catalogue
+    in a bin is DD/N_D^2 - 2 DR/(N_D N_R) + RR/N_R^2.  DD, RR (separate graphs) and DR (combined minus both) are
+    integer counts from the unweighted path, so this pins the signed fp64 path -- where the terms cancel to a few
+    per cent of their size -- by exact integers.  The 3pCF of the combined catalogue against the oracle, judged on
+    the A-13 scale sum |prod w|."""
+    from paper_2607_06604_b200 import estimators as est
+    d = cat.config2_data(seed=2105, n=20_000, L=270.0, mean_parents=200.0)
+    r = cat.config2_randoms(seed=2106, n=30_000, L=270.0)
+    nd, nr = d["points"].shape[0], r["points"].shape[0]
+    pts, w, wr = est.combined_catalogue(d["points"], r["points"])
+    assert abs(w[:nd].sum() - 1.0) < 1e-12 and abs(w[nd:].sum() + 1.0) < 1e-12
+    box, rmin, rmax, nb = d["box"], d["r_min"], d["r_max"], d["nbins"]
+    gd = gr.gramsci_build_graph(d["points"], None, box, rmin, rmax, nb)
+    grr = gr.gramsci_build_graph(r["points"], None, box, rmin, rmax, nb)
+    gc = gr.gramsci_build_graph(pts, w, box, rmin, rmax, nb)
+    dd, rr = gd.pcf2()[0], grr.pcf2()[0]
+    cc, nn = gc.pcf2(weighted=True)
+    dr = cc - dd - rr
+    want = dd / nd ** 2 - dr / (nd * nr) + rr / nr ** 2
+    scale = dd / nd ** 2 + dr / (nd * nr) + rr / nr ** 2              # sum |w_i w_j|
+    assert np.all(np.abs(want[-5:]) < 0.1 * scale[-5:])                  # at large r the terms cancel to a few per cent
+    assert np.all(np.abs(nn - want) <= 1e-10 * scale)
+    xi = est.signed_ratio(nn, rr / nr ** 2)
+    assert np.all(xi[:4] > 1.0)                                          # a clustered catalogue: xi >> 0 at small r
+    # triplets: combined signed catalogue against the oracle (sum |prod w| from the |w| run)
+    og = oracle.Graph(pts, w, box, rmin, rmax, nb)
+    oa = oracle.Graph(pts, np.abs(w), box, rmin, rmax, nb)
+    c3, n3 = gc.pcf3(weighted=True)
+    assert np.array_equal(c3, og.pcf3()[0])
+    assert_weighted_close(n3, og.pcf3()[1], scale=oa.pcf3()[1])
+
+
+@pytest.mark.slow
+def test_estimators_on_poisson_catalogues_at_full_size():
+    """configs[1] / configs[2] shapes through the estimator layer on the GPU path, Poisson data so that the truth is
+    known: (i) the combined 2e6-point signed catalogue (uniform "data" + uniform randoms in the configs[1] box): NNN/RRR
+    = 0 within shot noise -- the cancellation stress of the fp64 weighted path at full size; (ii) configs[2] points as
+    data + an equal-size random catalogue: NNNN/RRRR (even channel), xi = NN/RR, zeta_disc from Eq. 4 and zeta_conn =
+    zeta - zeta_disc (Eq. 5) all consistent with 0."""
+    from paper_2607_06604_b200 import estimators as est
+    torch = _torch()
+    # (i) 3pCF, 1e6 + 1e6 points, r < 30, 15 bins
+    d = cat.config2_randoms(seed=2201)
+    r = cat.config2_randoms(seed=2202)
+    nr = r["points"].shape[0]
+    pts, w, _ = est.combined_catalogue(d["points"], r["points"])
+    box, rmin, rmax, nb = d["box"], d["r_min"], d["r_max"], d["nbins"]
+    gc = gr.gramsci_build_graph(torch.from_numpy(pts).cuda(), torch.from_numpy(w).cuda(), box, rmin, rmax, nb)
+    grr = gr.gramsci_build_graph(torch.from_numpy(r["points"]).cuda(), None, box, rmin, rmax, nb)
+    c3, nnn = gc.pcf3(weighted=True)
+    rrr = grr.pcf3()[0] / float(nr) ** 3
+    gc.free(); grr.free()
+    ok = rrr * float(nr) ** 3 > 1e5
+    zeta = est.signed_ratio(nnn, rrr)
+    # a signed triple sum is a sum of ~8x as many +-terms as RRR has triangles; its noise is ~ a few / sqrt(RRR)
+    assert ok.sum() > 300 and np.all(np.abs(zeta[ok]) < 60.0 / np.sqrt(rrr[ok] * float(nr) ** 3))
+    assert c3.sum() > 7.5e9                                              # ~8x the triangles of one catalogue
+    # (ii) 4pCF, configs[2] + randoms
+    d = cat.config3()
+    r = cat.config3(seed=3002)
+    nr = r["points"].shape[0]
+    pts, w, _ = est.combined_catalogue(d["points"], r["points"])
+    box, rmin, rmax, nb = d["box"], d["r_min"], d["r_max"], d["nbins"]
+    gc = gr.gramsci_build_graph(torch.from_numpy(pts).cuda(), torch.from_numpy(w).cuda(), box, rmin, rmax, nb)
+    grr = gr.gramsci_build_graph(torch.from_numpy(r["points"]).cuda(), None, box, rmin, rmax, nb)
+    c4, nnnn = gc.pcf4(weighted=True)
+    rc4 = grr.pcf4()[0]
+    nn = gc.pcf2(weighted=True)[1]
+    rc2 = grr.pcf2()[0]
+    rr = rc2 / float(nr) ** 2
+    rrrr = rc4 / float(nr) ** 4
+    xi = est.signed_ratio(nn, rr)
+    assert np.all(np.abs(xi) < 8.0 / np.sqrt(rc2))                      # DD - 2DR + RR: shot noise ~ 2 / sqrt(RR)
+    zeta = est.signed_ratio(nnnn, rrrr)
+    zconn = est.zeta4_connected(np.nan_to_num(zeta), xi)
+    ok = rc4 > 2e5
+    assert ok.sum() > 500 and c4.sum() > 2e10
+    assert np.all(np.abs(zeta[ok]) < 100.0 / np.sqrt(rc4[ok]))
+    assert np.all(np.abs(zconn[ok]) < 100.0 / np.sqrt(rc4[ok]) + 1e-4)
