@@ -5,14 +5,15 @@ SURVEY.md 8(d), the end-to-end leg through host buffers and the CPU oracle timed
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2|cfg5|...]
                   [--subs cfg5,cfg5cap,cfg3,cfg4|none] [--scaling strong|weak]
 
-HEADLINE (the line's `value`, timed for exactly K steps after W warm-ups): BASELINE.json configs[1] ("cfg2": 1e6
-weighted Neyman-Scott points + 1e6 uniform randoms, r < 30, 15 bins).  A step is one pass of the whole hot path over
-the batch: for both catalogues, graph build (cell list, count, scan, fill; S:8(a) A1-A5) + 3pCF enumeration + fold
-(A7, A10), through the C ABI.  configs[1] is the headline because the driver times K = 20 steps: a step of the largest
-configuration (configs[4], 8.4e9 edges) takes ~18 s.  configs[4] -- the workload BASELINE's target sentence is
-about -- and configs[2], configs[3] are carried as COMPLETE SUB-RECORDS in the same line (`config.sub_records`), each
-with its own value, roofline, e2e and cpu_baseline, timed with CUDA events for one step:
-  cfg5     configs[4] with the whole graph resident      cfg5cap  the same under a 24 GiB device-memory cap (tiler)
+HEADLINE (the line's `value`, timed for exactly K steps after W warm-ups): BASELINE.json configs[4] ("cfg5": the
+BAO-scale 3pCF, 2.5e6 uniform points, 60 <= r < 150, 18 bins, 8.4e9 edges, 7.1e12 triangles, graph resident in HBM) --
+BASELINE.json's `metric` names no configuration, so the largest single-GPU one counts, and it is the workload the
+target sentence is about.  A step is one pass of the whole hot path over the batch: graph build (cell list, count,
+scan, fill; S:8(a) A1-A5) + 3pCF enumeration + fold (A7, A10), through the C ABI; ~17 s per step.
+The other configurations are carried as COMPLETE SUB-RECORDS in the same line (`config.sub_records`), each with its own
+value, roofline, e2e and cpu_baseline, timed with CUDA events:
+  cfg5cap  configs[4] under a 24 GiB device-memory cap (out-of-core tiler; `ooc_overhead` against the headline)
+  cfg2     configs[1]: 1e6 weighted Neyman-Scott points + 1e6 uniform randoms (build + 3pCF of both catalogues)
   cfg3     configs[2]: 4pCF + the 2pCF of the same graph  cfg4     configs[3]: weighted parity-4pCF
 L2: flushed between timed steps (256 MiB write); configs[4]'s 108 GB of graph exceed the 126 MB L2 by themselves.
 
@@ -21,8 +22,9 @@ dominant enumeration launch; `bound` names the term that won.  BW_HBM = MEASURED
 rate (the 4pCF bound) are MEASURED IN THIS RUN by bench_peaks.cu (built into libbench_peaks.so) -- no constants.
 `traffic` = DRAM bytes of one launch of that kernel from the committed ncu capture named in `traffic_source`.
 
-N > 1 (torchrun): by default the hubs of ONE workload are sharded over the ranks (strong scaling; every rank builds the
-graph, one all-reduce of the histogram -- S:8(e)); per-rank enumeration times and their imbalance are reported.
+N > 1 (torchrun): by default the hubs of ONE workload are sharded over the ranks (strong scaling): every rank builds
+the SLAB + HALO part of the graph it needs (gramsci_options.slab_count; --partition modulo keeps the whole graph on every
+rank), one all-reduce of the histogram -- S:8(e); per-rank enumeration times and their imbalance are reported.
 --scaling weak gives every rank its own catalogues instead.  --impl reference times the CPU oracle.
 """
 from __future__ import annotations
@@ -190,6 +192,8 @@ def workload(name: str, seed_shift: int = 0):
         return [cat.config1(seed=1001 + seed_shift)]
     if name == "cfg5p":       # scaled replica of configs[4] (same density, L=425)
         return [cat.config5(seed=5001 + seed_shift, n=39_062, L=425.0)]
+    if name == "cfg5e":       # 1/8 replica of configs[4] (same density, L=850): the long-row kernel's profiling case
+        return [cat.config5(seed=5001 + seed_shift, n=312_500, L=850.0)]
     if name in ("cfg5", "cfg5cap"):   # configs[4] in full: 2.5e6 points, 8.4e9 edges, 42 GB of CSR
         return [cat.config5(seed=5001 + seed_shift)]
     if name == "cfg3":        # configs[2]: 4pCF (+ the 2pCF of the same graph for the disconnected term)
@@ -223,7 +227,7 @@ def oracle_sample(name: str, cats, budget_s: float = 8.0):
     for c in cats:
         kind = c["kind"]
         n = c["points"].shape[0]
-        if name in ("cfg5", "cfg5cap", "cfg5p") and n > 100_000:
+        if name in ("cfg5", "cfg5cap", "cfg5p", "cfg5e") and n > 100_000:
             # rows found on demand from the cell list (the graph is too large to hold): sampled hubs
             g = oracle.Graph(c["points"], c["weights"], c["box"], c["r_min"], c["r_max"], c["nbins"], lists=False)
             hubs = np.arange(0, n, n // 48)[:48]
@@ -302,6 +306,16 @@ class Runner:
                     for c in cats]
         self.stats = {}
 
+    def partition(self):
+        """Strong scaling: which tuples this rank enumerates.  'slab' (default for spatially labelled graphs): slab + halo
+        -- the rank stores only the rows of its slab of cells and of their forward stencil (S:8(e), P:251-253);
+        'modulo': every rank holds the whole graph and takes the hubs with label % world == rank."""
+        if not self.strong:
+            return {}
+        if self.args.partition == "slab" and self.cats[0]["kind"] != "4pcf_parity":
+            return dict(slab_count=self.world, slab_index=self.rank)
+        return dict(shard_count=self.world, shard_index=self.rank)
+
     def step(self, host: bool, count_work: bool = False):
         """One pass of the hot path over the batch: (tuples, step stats, per-catalogue stats)."""
         import paper_2607_06604_b200 as gr
@@ -314,7 +328,7 @@ class Runner:
             kind = c["kind"]
             g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=self.args.algo,
                                        want_pixels=(kind == "4pcf_parity"), device_mem_cap_bytes=int(self.cap * 2 ** 30),
-                                       shard_count=self.world if self.strong else 0, shard_index=self.rank if self.strong else 0)
+                                       **self.partition())
             st["build_ms"] += g.timing(0)
             st["launches"] += g.timing(3)
             pc = {"name": c["name"], "weighted": w is not None, "kind": kind}
@@ -502,24 +516,27 @@ def run_ours(args):
         sampler.start()
         time.sleep(0.3)
     big = args.workload in ("cfg5", "cfg5cap", "cfg4")
+    # e2e leg: half the steps, at most 3 for the workloads whose step takes ~17 s
+    e2e_steps = 0 if args.skip_e2e else max(1, min(args.steps // 2, 3 if big else args.steps))
     rec = record_for(args.workload, cats, args, peaks, hbm, hbm_kind, flush, args.steps, args.warmup,
-                     0 if args.skip_e2e else max(1, args.steps // 2), world, rank, strong,
-                     with_cpu=not args.no_cpu_baseline)
+                     e2e_steps, world, rank, strong, with_cpu=not args.no_cpu_baseline)
     clocks = sampler.stop() if rank == 0 else None
 
     subs = {}
-    if rank == 0 and world == 1 and args.subs != "none" and not big:
-        for name in [s for s in args.subs.split(",") if s]:
+    if rank == 0 and world == 1 and args.subs != "none":
+        for name in [s for s in args.subs.split(",") if s and s != args.workload]:
             torch.cuda.synchronize()
             gr.gramsci_release_memory()
-            # one timed step (an 18 s step does not warm up; the first step of cfg5 also pays the growth of the memory
-            # pool to 108 GB); the capped run's overhead is taken against the resident run of this same process
-            sub = record_for(name, workload(name), args, peaks, hbm, hbm_kind, flush, 1, 0 if name != "cfg3" else 3,
-                             0 if args.skip_e2e else 1, with_cpu=not args.no_cpu_baseline)
+            # small workloads: 5 timed steps after 3 warm-ups; the ~17 s ones: one timed step after one warm-up (as warm
+            # as the headline's steps: memory pool grown, host blocks of the capped build page-locked once)
+            small = name in ("cfg2", "cfg3", "cfg1")
+            sub = record_for(name, workload(name), args, peaks, hbm, hbm_kind, flush, 5 if small else 1, 3 if small else 1,
+                             0 if args.skip_e2e else (2 if small else 1), with_cpu=not args.no_cpu_baseline)
             sub.pop("data", None)
             subs[name] = sub
-        if "cfg5" in subs and "cfg5cap" in subs:
-            a, b = subs["cfg5"], subs["cfg5cap"]
+        res = rec if args.workload == "cfg5" else subs.get("cfg5")
+        if res is not None and "cfg5cap" in subs:
+            a, b = res, subs["cfg5cap"]
             b["config"]["ooc_overhead"] = {
                 "query": b["config"]["query_ms"] / a["config"]["query_ms"] - 1.0,
                 "build_plus_query": (b["config"]["build_ms"] + b["config"]["query_ms"]) / (a["config"]["build_ms"] + a["config"]["query_ms"]) - 1.0,
@@ -538,9 +555,9 @@ def run_ours(args):
         "config": dict(rec["config"], algo=args.algo,
                        step="graph build + enumeration (3pCF / 4pCF / parity-4pCF by workload) + fold for every catalogue",
                        l2="flushed between timed steps (256 MiB write); every workload's graph also exceeds the 126 MB L2",
-                       headline_note="BASELINE.json names no configuration for its metric; configs[1] is the headline because "
-                       "the driver times K = 20 steps and a step of configs[4] takes ~18 s; configs[4] (resident and "
-                       "under a 24 GiB cap), configs[2] and configs[3] are complete sub-records below",
+                       headline_note="BASELINE.json names no configuration for its metric, so the largest single-GPU one "
+                       "(configs[4], the 8.4e9-edge BAO-scale 3pCF the target sentence is about) is the headline; the same "
+                       "under a 24 GiB cap, configs[1], configs[2] and configs[3] are complete sub-records below",
                        peaks_measured_in_run=peaks, sub_records=subs),
         "clocks": clocks, "e2e": rec["e2e"], "gpu_launches": rec["gpu_launches"], "roofline": rec["roofline"],
     }
@@ -557,14 +574,16 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2")
-    ap.add_argument("--subs", default="cfg5,cfg5cap,cfg3,cfg4",
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--subs", default="cfg5cap,cfg2,cfg3,cfg4",
                     help="sub-records carried in the line at N = 1 (comma list of workloads, or 'none')")
     ap.add_argument("--algo", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scaling", default="strong", choices=["weak", "strong"],
                     help="N > 1: strong (default) = the hubs of ONE workload sharded over the ranks, histograms all-reduced; "
                          "weak = every rank its own catalogues")
+    ap.add_argument("--partition", default="slab", choices=["slab", "modulo"],
+                    help="strong scaling: slab + halo graph per rank (default), or whole graph per rank with hubs label %% N")
     ap.add_argument("--skip-e2e", action="store_true", help="no host-buffer leg (e2e = null)")
     ap.add_argument("--cap-gib", type=float, default=0.0,
                     help="device_mem_cap_bytes in GiB (0 = whole CSR resident); forces the out-of-core tiler")

@@ -101,6 +101,16 @@ typedef struct {       /* zero-initialised struct == defaults */
                                       shard_index.  The shards partition the tuples: the histograms of shards
                                       0..shard_count-1 add up to the full result, exactly for counts -- one GPU
                                       per shard and one all-reduce of the histogram (S:8(e)); 2pCF is not sharded */
+    int slab_count, slab_index;    /* slab_count > 1 (spatial labels only): SLAB + HALO partition for one GPU per slab
+                                      (S:8(e), "one hub window per device ... no communication between
+                                      tiles").  The cells (in id order = z-slabs of the grid) are cut into slab_count
+                                      contiguous ranges of equal estimated work (sum of squared row lengths); this
+                                      graph OWNS the hubs of range slab_index and stores only the rows of its own
+                                      cells and of the cells its hubs' neighbours lie in (the forward stencil: the
+                                      halo) -- every other row is empty, so memory is ~1/slab_count + halo.  All
+                                      slabs must be built from the same points in the same order.  The histograms of
+                                      the slabs add up to the full result (exactly for counts): one all-reduce.
+                                      2pCF counts the edges stored at owned hubs.  Not combinable with shard_count */
     int reserved;                  /* must be 0 */
     /* Device allocator hooks (S:8(b)): both or neither.  alloc returns a DEVICE pointer valid on `stream`
        (256-byte aligned) or NULL; dealloc releases it.  NULL = the library's private memory pool.       */
@@ -127,7 +137,8 @@ int gramsci_build_graph(const double *points, const double *weights, int64_t N, 
                         double r_min, double r_max, int nbins, const gramsci_options *opt,
                         gramsci_graph **out);
 
-/* Sizes of a built graph (all out-pointers HOST, any may be NULL). csr_bytes = 5E (+E with pixels). */
+/* Sizes of a built graph (all out-pointers HOST, any may be NULL). csr_bytes = 5E (+E with pixels).
+ * n_edges counts the STORED edges (a slab graph stores the rows of its slab and halo only). */
 int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edges, int32_t *max_row,
                        uint64_t *csr_bytes, int32_t *n_windows);
 
@@ -191,6 +202,10 @@ int gramsci_last_timing(const gramsci_graph *g, int what, double *value);
 /* Exact work counters of the 3pCF on this graph (device pre-pass; S:8(d)): spoke_elems = sum over
  * oriented edges (i,j) of len(N+(j)); tail_elems = sum of len(tail_i(j)).  HOST out-pointers. */
 int gramsci_work_counters(const gramsci_graph *g, uint64_t *spoke_elems, uint64_t *tail_elems);
+
+/* The hubs a graph owns, as a range [hub_lo, hub_hi) of INTERNAL labels (out-pointers HOST): the whole catalogue
+ * [0, N) unless the graph was built with slab_count > 1. */
+int gramsci_slab_range(const gramsci_graph *g, int32_t *hub_lo, int32_t *hub_hi);
 
 void gramsci_free_graph(gramsci_graph *g);
 

@@ -25,7 +25,7 @@ ABI_SYMBOLS = [
     "gramsci_build_graph", "gramsci_graph_info", "gramsci_export_csr", "gramsci_2pcf", "gramsci_3pcf",
     "gramsci_4pcf", "gramsci_4pcf_parity", "gramsci_num_configs", "gramsci_compact", "gramsci_zeta_disc",
     "gramsci_last_timing", "gramsci_work_counters", "gramsci_free_graph", "gramsci_last_error",
-    "gramsci_export_labels", "gramsci_release_memory", "gramsci_3pcf_equilateral",
+    "gramsci_export_labels", "gramsci_release_memory", "gramsci_3pcf_equilateral", "gramsci_slab_range",
 ]
 
 ALGO_DEFAULT, ALGO_MERGEPATH, ALGO_BSEARCH, ALGO_BITMAP = 0, 1, 2, 3
@@ -50,7 +50,8 @@ class _Options(ctypes.Structure):
     _fields_ = [("stream", ctypes.c_void_p), ("device_mem_cap_bytes", ctypes.c_uint64),
                 ("want_pixels", ctypes.c_int), ("relabel", ctypes.c_int), ("algo", ctypes.c_int),
                 ("n_windows", ctypes.c_int), ("hub_stride", ctypes.c_int),
-                ("shard_count", ctypes.c_int), ("shard_index", ctypes.c_int), ("reserved", ctypes.c_int),
+                ("shard_count", ctypes.c_int), ("shard_index", ctypes.c_int),
+                ("slab_count", ctypes.c_int), ("slab_index", ctypes.c_int), ("reserved", ctypes.c_int),
                 ("alloc", _ALLOC_FN), ("dealloc", _DEALLOC_FN), ("user", ctypes.c_void_p)]
 
 
@@ -115,6 +116,8 @@ def load_library():
     L.gramsci_export_labels.argtypes = [vp, vp]
     L.gramsci_release_memory.restype = ctypes.c_int
     L.gramsci_release_memory.argtypes = []
+    L.gramsci_slab_range.restype = ctypes.c_int
+    L.gramsci_slab_range.argtypes = [vp, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
     _lib = L
     return L
 
@@ -168,6 +171,12 @@ class Graph:
         _check(load_library().gramsci_graph_info(self._h, ctypes.byref(n), ctypes.byref(e), ctypes.byref(mr),
                                                  ctypes.byref(cb), ctypes.byref(nw)))
         return dict(n_points=n.value, n_edges=e.value, max_row=mr.value, csr_bytes=cb.value, n_windows=nw.value)
+
+    def slab_range(self):
+        """``gramsci_slab_range``: the hubs this graph owns, [hub_lo, hub_hi) in internal labels."""
+        lo, hi = ctypes.c_int32(), ctypes.c_int32()
+        _check(load_library().gramsci_slab_range(self._h, ctypes.byref(lo), ctypes.byref(hi)))
+        return lo.value, hi.value
 
     def timing(self, what: int) -> float:
         v = ctypes.c_double()
@@ -253,7 +262,8 @@ class Graph:
 def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = None, r_min: float = 0.0,
                         r_max: float = 1.0, nbins: int = 1, *, want_pixels: bool = False, relabel: int = 0,
                         algo: int = 0, device_mem_cap_bytes: int = 0, n_windows: int = 0, hub_stride: int = 0,
-                        shard_count: int = 0, shard_index: int = 0, torch_allocator: bool = False) -> Graph:
+                        shard_count: int = 0, shard_index: int = 0, slab_count: int = 0, slab_index: int = 0,
+                        torch_allocator: bool = False) -> Graph:
     """``gramsci_build_graph`` (include/gramsci.h).  ``points`` [N,3] / ``weights`` [N] fp64: torch CUDA
     tensors (used in place), torch CPU tensors or NumPy arrays (the library stages host buffers itself)."""
     L = load_library()
@@ -280,6 +290,8 @@ def gramsci_build_graph(points, weights=None, box: Optional[Sequence[float]] = N
     opt.hub_stride = int(hub_stride)
     opt.shard_count = int(shard_count)
     opt.shard_index = int(shard_index)
+    opt.slab_count = int(slab_count)
+    opt.slab_index = int(slab_index)
     if torch_allocator:          # S:8(b): the graph and all scratch come from torch's caching allocator
         opt.alloc, opt.dealloc = _TORCH_HOOKS
     cbox = None

@@ -113,6 +113,7 @@ extern "C" int gramsci_release_memory(void)
         GR_CUDA(cudaDeviceSynchronize());
         GR_CUDA(cudaMemPoolTrimTo(pool, 0));
     }
+    gr_pinned_release_cache();
     GR_API_END
 }
 
@@ -148,11 +149,33 @@ int gr_kernel_occupancy(const void *fn, int threads, size_t smem)
 }
 
 // ---- page-locked host memory -------------------------------------------------------------------------------
-void *gr_pinned_alloc(size_t bytes)
+namespace {
+struct PinnedBlock { void *p; size_t bytes; };
+std::mutex g_pin_mu;
+std::vector<PinnedBlock> g_pin_cache;
+}
+
+void *gr_pinned_alloc_nothrow(size_t *bytes_io, std::string *err)
 {
-    bytes = (bytes + 4095) & ~size_t(4095);
+    size_t bytes = (*bytes_io + 4095) & ~size_t(4095);
+    {   // smallest cached block that fits without wasting more than half of it
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        int best = -1;
+        for (int k = 0; k < (int)g_pin_cache.size(); ++k)
+            if (g_pin_cache[k].bytes >= bytes && g_pin_cache[k].bytes <= 2 * bytes + (size_t(1) << 20) &&
+                (best < 0 || g_pin_cache[k].bytes < g_pin_cache[best].bytes)) best = k;
+        if (best >= 0) {
+            PinnedBlock b = g_pin_cache[best];
+            g_pin_cache.erase(g_pin_cache.begin() + best);
+            *bytes_io = b.bytes;
+            return b.p;
+        }
+    }
     void *p = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
-    if (p == MAP_FAILED) GR_FAIL(GRAMSCI_ENOMEM, "out-of-core: cannot map %zu bytes of host memory", bytes);
+    if (p == MAP_FAILED) {
+        if (err) *err = "out-of-core: cannot map " + std::to_string(bytes) + " bytes of host memory";
+        return nullptr;
+    }
     madvise(p, bytes, MADV_HUGEPAGE);
     unsigned nt = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
     if (bytes < (size_t(64) << 20)) nt = 1;
@@ -169,17 +192,40 @@ void *gr_pinned_alloc(size_t bytes)
     if (e != cudaSuccess) {
         munmap(p, bytes);
         cudaGetLastError();
-        GR_FAIL(GRAMSCI_ENOMEM, "out-of-core: cannot page-lock %zu bytes of host memory (%s)", bytes, cudaGetErrorString(e));
+        if (err) *err = "out-of-core: cannot page-lock " + std::to_string(bytes) + " bytes of host memory (" + cudaGetErrorString(e) + ")";
+        return nullptr;
     }
+    *bytes_io = bytes;
+    return p;
+}
+
+void *gr_pinned_alloc(size_t *bytes)
+{
+    std::string err;
+    void *p = gr_pinned_alloc_nothrow(bytes, &err);
+    if (!p) GR_FAIL(GRAMSCI_ENOMEM, "%s", err.c_str());
     return p;
 }
 
 void gr_pinned_free(void *p, size_t bytes)
 {
     if (!p) return;
-    bytes = (bytes + 4095) & ~size_t(4095);
-    cudaHostUnregister(p);
-    munmap(p, bytes);
+    std::lock_guard<std::mutex> lk(g_pin_mu);
+    g_pin_cache.push_back({p, (bytes + 4095) & ~size_t(4095)});
+}
+
+void gr_pinned_release_cache()
+{
+    std::vector<PinnedBlock> blocks;
+    {
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        blocks.swap(g_pin_cache);
+    }
+    for (auto &b : blocks) {
+        cudaHostUnregister(b.p);
+        munmap(b.p, b.bytes);
+    }
+    cudaGetLastError();
 }
 
 // ---- pointer staging -------------------------------------------------------------------------------------
@@ -259,7 +305,9 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     memset(&o, 0, sizeof o);
     if (opt) o = *opt;
     if (o.relabel < 0 || o.relabel > 2 || o.algo < 0 || o.algo > GRAMSCI_ALGO_MAX || o.n_windows < 0 || o.hub_stride < 0 ||
-        o.shard_count < 0 || o.shard_index < 0 || (o.shard_count > 1 && o.shard_index >= o.shard_count))
+        o.shard_count < 0 || o.shard_index < 0 || (o.shard_count > 1 && o.shard_index >= o.shard_count) ||
+        o.slab_count < 0 || o.slab_index < 0 || (o.slab_count > 1 && o.slab_index >= o.slab_count) ||
+        (o.slab_count > 1 && o.shard_count > 1))
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: bad options");
     require_device();
 
@@ -293,6 +341,12 @@ extern "C" int gramsci_build_graph(const double *points, const double *weights, 
     g->hub_stride = o.hub_stride > 1 ? o.hub_stride : 1;
     g->shard_count = o.shard_count > 1 ? o.shard_count : 1;
     g->shard_index = o.shard_count > 1 ? o.shard_index : 0;
+    g->slab_count = o.slab_count > 1 ? o.slab_count : 1;
+    g->slab_index = o.slab_count > 1 ? o.slab_index : 0;
+    if (g->slab_count > 1 && !g->spatial) {
+        delete g; g = nullptr;
+        GR_FAIL(GRAMSCI_EINVAL, "build_graph: slab_count needs spatial (cell-order) labels: not with want_pixels / relabel = 2");
+    }
     if (g->has_pix && g->spatial) {
         delete g; g = nullptr;
         GR_FAIL(GRAMSCI_EINVAL, "build_graph: want_pixels needs caller labels (A-10): relabel = 1 cannot be combined with it");
@@ -340,9 +394,7 @@ extern "C" void gramsci_free_graph(gramsci_graph *g)
 {
     if (!g) return;
     cudaStreamSynchronize(g->stream);
-    gr_pinned_free(g->h_idx, g->h_idx_bytes);
-    gr_pinned_free(g->h_bin, g->h_bin_bytes);
-    gr_pinned_free(g->h_pix, g->h_pix_bytes);
+    for (auto &w : g->windows) { gr_pinned_free(w.h_block, w.h_block_bytes); w.h_block = nullptr; }
     const bool big = (uint64_t)g->n_edges * 5 > ((uint64_t)4 << 30) && !g->actx.alloc;
     cudaStream_t st = g->stream;
     delete g;
@@ -355,6 +407,15 @@ extern "C" void gramsci_free_graph(gramsci_graph *g)
         }
         cudaGetLastError();
     }
+}
+
+extern "C" int gramsci_slab_range(const gramsci_graph *g, int32_t *hub_lo, int32_t *hub_hi)
+{
+    GR_API_BEGIN
+    if (!g) GR_FAIL(GRAMSCI_EINVAL, "slab_range: graph is NULL");
+    if (hub_lo) *hub_lo = std::max(0, g->hub_lo);
+    if (hub_hi) *hub_hi = (int32_t)std::min<int64_t>(g->n, g->hub_hi);
+    GR_API_END
 }
 
 extern "C" int gramsci_graph_info(const gramsci_graph *g, int64_t *n_points, int64_t *n_edges, int32_t *max_row,

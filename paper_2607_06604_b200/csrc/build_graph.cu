@@ -16,6 +16,10 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <atomic>
+#include <chrono>
+#include <string>
+#include <thread>
 
 namespace {
 
@@ -368,7 +372,10 @@ k_neighbours(const __grid_constant__ BuildParams c_bp, const __grid_constant__ B
     if (keep) { cs = cell_start[id]; ce = cell_start[id + 1]; }
 
     int64_t out = 0;
-    if (FILL) out = ptr[li] - e0;
+    if (FILL) {
+        out = ptr[li] - e0;
+        if (ptr[li + 1] == ptr[li]) return;             // empty row (also: a row outside slab + halo of a slab graph)
+    }
     int count = 0;
     // The (cell, 32-candidate chunk) pairs are walked as one sequence with the NEXT chunk's label and
     // coordinates already in flight while the current chunk's distances are evaluated (a cell holds about one
@@ -450,6 +457,23 @@ k_neighbours(const __grid_constant__ BuildParams c_bp, const __grid_constant__ B
         }
     }
     if (!FILL && lane == 0) deg[li] = count;
+}
+
+// ---- slab + halo partition (S:8(e)): work estimate per cell, rows of cells outside slab + halo emptied ----
+__global__ void k_cell_cost(int64_t ncell, const int32_t *__restrict__ cell_start, const int32_t *__restrict__ deg,
+                            double *__restrict__ cost)
+{
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    double s = 0.0;
+    for (int i = cell_start[c]; i < cell_start[c + 1]; ++i) s += (double)deg[i] * (double)deg[i];
+    cost[c] = s;
+}
+
+__global__ void k_mask_deg(int64_t n, const int32_t *__restrict__ cell_of, const uint8_t *__restrict__ keep, int32_t *__restrict__ deg)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && !keep[cell_of[i]]) deg[i] = 0;
 }
 
 // ---- export in caller labels (spatial mode): re-orient every edge to lower caller label ---------------
@@ -765,6 +789,51 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
     const unsigned nblk = blocks_for(n * 32, 256);
     k_neighbours<false><<<nblk, 256, 0, st>>>(bp, eq, sx.p, sy.p, sz.p, lab.p, cell_start.p, 0, n, 0, INT32_MAX, deg.p,
                                               nullptr, 0, nullptr, nullptr, nullptr);
+    if (g->slab_count > 1) {
+        // equal-work cell ranges (work of a hub ~ its wedges ~ deg^2); this graph owns range slab_index and keeps the
+        // rows of its cells and of their forward stencil cells (where the spokes of its hubs live)
+        DevBuf<double> cost;
+        cost.alloc((size_t)ncell);
+        k_cell_cost<<<blocks_for(ncell, 128), 128, 0, st>>>(ncell, cell_start.p, deg.p, cost.p);
+        std::vector<double> hc((size_t)ncell);
+        std::vector<int32_t> hs((size_t)ncell + 1);
+        GR_CUDA(cudaMemcpyAsync(hc.data(), cost.p, sizeof(double) * ncell, cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaMemcpyAsync(hs.data(), cell_start.p, sizeof(int32_t) * (ncell + 1), cudaMemcpyDeviceToHost, st));
+        GR_CUDA(cudaStreamSynchronize(st));
+        double total = 0.0;
+        for (double x : hc) total += x + 1.0;           // + 1 per cell: empty catalogues still split
+        auto boundary = [&](int k) -> int64_t {          // first cell of range k
+            if (k <= 0) return 0;
+            if (k >= g->slab_count) return ncell;
+            const double want = total * (double)k / (double)g->slab_count;
+            double acc = 0.0;
+            for (int64_t c = 0; c < ncell; ++c) { if (acc >= want) return c; acc += hc[c] + 1.0; }
+            return ncell;
+        };
+        const int64_t c_lo = boundary(g->slab_index), c_hi = boundary(g->slab_index + 1);
+        std::vector<uint8_t> keep((size_t)ncell, 0);
+        for (int64_t c = c_lo; c < c_hi; ++c) {
+            const int cx = (int)(c % g->nc[0]), cy = (int)((c / g->nc[0]) % g->nc[1]), cz = (int)(c / ((int64_t)g->nc[0] * g->nc[1]));
+            for (int t = 0; t < 27; ++t) {
+                int o[3] = {cx + (t % 3) - 1, cy + ((t / 3) % 3) - 1, cz + (t / 9) - 1};
+                bool ok = true;
+                for (int a = 0; a < 3; ++a) {
+                    if (g->periodic) o[a] = (o[a] + g->nc[a]) % g->nc[a];
+                    else if (o[a] < 0 || o[a] >= g->nc[a]) ok = false;
+                }
+                if (!ok) continue;
+                const int64_t id = ((int64_t)o[2] * g->nc[1] + o[1]) * g->nc[0] + o[0];
+                if (id >= c) keep[(size_t)id] = 1;
+            }
+        }
+        g->cell_keep.alloc((size_t)ncell);
+        GR_CUDA(cudaMemcpyAsync(g->cell_keep.p, keep.data(), (size_t)ncell, cudaMemcpyHostToDevice, st));
+        k_mask_deg<<<blocks_for(n, 256), 256, 0, st>>>(n, g->cell_of.p, g->cell_keep.p, deg.p);
+        GR_CUDA(cudaStreamSynchronize(st));             // `keep` goes out of scope
+        g->hub_lo = hs[(size_t)c_lo];
+        g->hub_hi = hs[(size_t)c_hi];
+        launches += 2;
+    }
     exclusive_scan<int64_t>(deg.p, n, g->ptr.p, st);
     launches += 4;
     int64_t E = 0;
@@ -849,23 +918,21 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         }
         GR_CUDA(cudaGetLastError());      // (row statistics of the slot-table kernel: on first use, gr_row_stats)
     } else {
-        g->h_idx_bytes = std::max<size_t>((size_t)E * 4 + 256, 256);
-        g->h_bin_bytes = std::max<size_t>((size_t)E + 256, 256);
-        g->h_idx = (int32_t *)gr_pinned_alloc(g->h_idx_bytes);
-        g->h_bin = (uint8_t *)gr_pinned_alloc(g->h_bin_bytes);
-        if (g->has_pix) {
-            g->h_pix_bytes = g->h_bin_bytes;
-            g->h_pix = (uint8_t *)gr_pinned_alloc(g->h_pix_bytes);
-        }
+        // Every window gets ONE page-locked host block [idx | bin | pix] (entry 0 = edge e_lo).  Page-locking is the
+        // slowest step of a capped build (~25 GiB/s on this box, 42 GB for configs[4]), so a background thread prepares
+        // the blocks in window order (cached blocks of an earlier graph first) while the device fills the windows;
+        // fills go to two staging buffers, and the copy of window k to the host (copy stream) overlaps the fill of k+1.
+        const int Wn = (int)g->windows.size();
+        if (Wn > 1024) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small: %d windows", Wn);
         int64_t maxlen = 0;
         for (auto &w : g->windows) maxlen = std::max(maxlen, w.e_hi - w.e_lo);
-        DevBuf<int32_t> widx;
-        DevBuf<uint8_t> wbin, wpix;
-        widx.alloc((size_t)maxlen); wbin.alloc((size_t)maxlen);
-        if (g->has_pix) wpix.alloc((size_t)maxlen);
-        const int Wn = (int)g->windows.size();
+        DevBuf<int32_t> widx[2];
+        DevBuf<uint8_t> wbin[2], wpix[2];
+        for (int k = 0; k < 2; ++k) {
+            widx[k].alloc((size_t)maxlen); wbin[k].alloc((size_t)maxlen);
+            if (g->has_pix) wpix[k].alloc((size_t)maxlen);
+        }
         g->need.assign((size_t)Wn * Wn, 0);
-        if (Wn > 1024) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small: %d windows", Wn);
         const int mwords = (Wn + 31) / 32;
         DevBuf<unsigned int> dmask;
         DevBuf<int32_t> dwlo;
@@ -879,38 +946,88 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
             GR_CUDA(cudaMemcpyAsync(dwlo.p, hw.data(), sizeof(int32_t) * (Wn + 1), cudaMemcpyHostToDevice, st));
             GR_CUDA(cudaStreamSynchronize(st));
         }
-        int hwin = 0;
-        for (auto &w : g->windows) {
+        struct Pipe {                                   // joined / destroyed before the staging buffers go away
+            std::thread th;
+            std::atomic<int> ready{0}, failed{0}, stop{0};
+            std::string err;
+            cudaStream_t cs = nullptr;
+            cudaEvent_t filled[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+            ~Pipe() {
+                stop.store(1);
+                if (th.joinable()) th.join();
+                if (cs) { cudaStreamSynchronize(cs); cudaStreamDestroy(cs); }
+                for (int k = 0; k < 2; ++k) { if (filled[k]) cudaEventDestroy(filled[k]); if (copied[k]) cudaEventDestroy(copied[k]); }
+            }
+        } pipe;
+        GR_CUDA(cudaStreamCreateWithFlags(&pipe.cs, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            GR_CUDA(cudaEventCreateWithFlags(&pipe.filled[k], cudaEventDisableTiming));
+            GR_CUDA(cudaEventCreateWithFlags(&pipe.copied[k], cudaEventDisableTiming));
+        }
+        int dev = 0;
+        GR_CUDA(cudaGetDevice(&dev));
+        const int has_pix = g->has_pix;
+        pipe.th = std::thread([g, Wn, dev, has_pix, &pipe] {
+            cudaSetDevice(dev);
+            for (int k = 0; k < Wn && !pipe.stop.load(); ++k) {
+                GrWindow &w = g->windows[k];
+                const size_t len = (size_t)(w.e_hi - w.e_lo);
+                const size_t sec_i = (len * 4 + 255) & ~size_t(255), sec_b = (len + 255) & ~size_t(255);
+                size_t bytes = std::max<size_t>(4096, sec_i + sec_b * (has_pix ? 2 : 1));
+                void *blk = gr_pinned_alloc_nothrow(&bytes, &pipe.err);
+                if (!blk) { pipe.failed.store(1); return; }
+                w.h_block = blk;
+                w.h_block_bytes = bytes;
+                w.h_idx = (int32_t *)blk;
+                w.h_bin = (uint8_t *)blk + sec_i;
+                w.h_pix = has_pix ? (uint8_t *)blk + sec_i + sec_b : nullptr;
+                pipe.ready.store(k + 1, std::memory_order_release);
+            }
+        });
+        for (int hwin = 0; hwin < Wn; ++hwin) {
+            GrWindow &w = g->windows[hwin];
+            const int sb = hwin & 1;
             int64_t len = w.e_hi - w.e_lo;
             int64_t s_lo = g->spatial ? w.row_lo : 0, s_hi = g->spatial ? w.row_hi : n;
             unsigned nb2 = blocks_for((s_hi - s_lo) * 32, 256);
+            if (hwin >= 2) GR_CUDA(cudaStreamWaitEvent(st, pipe.copied[sb], 0));     // window hwin-2 has left this staging buffer
             k_neighbours<true><<<nb2, 256, 0, st>>>(bp, eq, sx.p, sy.p, sz.p, lab.p, cell_start.p, s_lo, s_hi, w.row_lo, w.row_hi,
-                                                    nullptr, g->ptr.p, w.e_lo, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr);
+                                                    nullptr, g->ptr.p, w.e_lo, widx[sb].p, wbin[sb].p, g->has_pix ? wpix[sb].p : nullptr);
             launches += 1;
             if (!g->spatial) {
-                segsort<int64_t>(g->ptr.p, w.row_lo, w.row_hi, w.e_lo, g->max_row, widx.p, wbin.p, g->has_pix ? wpix.p : nullptr, st);
+                segsort<int64_t>(g->ptr.p, w.row_lo, w.row_hi, w.e_lo, g->max_row, widx[sb].p, wbin[sb].p, g->has_pix ? wpix[sb].p : nullptr, st);
                 launches += 1;
             }
-            k_row_stats<<<blocks_for((int64_t)(w.row_hi - w.row_lo) * 32, 256), 256, 0, st>>>(g->ptr.p, widx.p, w.e_lo,
+            GR_CUDA(cudaEventRecord(pipe.filled[sb], st));
+            k_row_stats<<<blocks_for((int64_t)(w.row_hi - w.row_lo) * 32, 256), 256, 0, st>>>(g->ptr.p, widx[sb].p, w.e_lo,
                                                                                            w.row_lo, w.row_hi, stats.p);
             launches += 1;
             int64_t head = hptr[w.row_lo] - w.e_lo;   // entries before the first row belong to the previous window
             // search windows this hub window reaches (exact)
             GR_CUDA(cudaMemsetAsync(dmask.p, 0, sizeof(unsigned int) * mwords, st));
             if (len > head)
-                k_need_mask<<<296, 256, sizeof(unsigned int) * mwords, st>>>(widx.p, head, len, dwlo.p, Wn, dmask.p);
+                k_need_mask<<<296, 256, sizeof(unsigned int) * mwords, st>>>(widx[sb].p, head, len, dwlo.p, Wn, dmask.p);
             GR_CUDA(cudaMemcpyAsync(hmask.data(), dmask.p, sizeof(unsigned int) * mwords, cudaMemcpyDeviceToHost, st));
-            GR_CUDA(cudaStreamSynchronize(st));
             launches += 1;
+            // the host block of this window (background thread), then its copy on the copy stream
+            while (pipe.ready.load(std::memory_order_acquire) <= hwin) {
+                if (pipe.failed.load()) GR_FAIL(GRAMSCI_ENOMEM, "%s", pipe.err.c_str());
+                std::this_thread::sleep_for(std::chrono::microseconds(50));
+            }
+            GR_CUDA(cudaStreamWaitEvent(pipe.cs, pipe.filled[sb], 0));
+            if (len > head) {
+                GR_CUDA(cudaMemcpyAsync(w.h_idx + head, widx[sb].p + head, (size_t)(len - head) * 4, cudaMemcpyDeviceToHost, pipe.cs));
+                GR_CUDA(cudaMemcpyAsync(w.h_bin + head, wbin[sb].p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, pipe.cs));
+                if (g->has_pix)
+                    GR_CUDA(cudaMemcpyAsync(w.h_pix + head, wpix[sb].p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, pipe.cs));
+            }
+            GR_CUDA(cudaEventRecord(pipe.copied[sb], pipe.cs));
+            GR_CUDA(cudaStreamSynchronize(st));
             for (int c = 0; c < Wn; ++c)
                 if (hmask[c >> 5] & (1u << (c & 31))) g->need[(size_t)hwin * Wn + c] = 1;
-            ++hwin;
-            GR_CUDA(cudaMemcpyAsync(g->h_idx + w.e_lo + head, widx.p + head, (size_t)(len - head) * 4, cudaMemcpyDeviceToHost, st));
-            GR_CUDA(cudaMemcpyAsync(g->h_bin + w.e_lo + head, wbin.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));
-            if (g->has_pix)
-                GR_CUDA(cudaMemcpyAsync(g->h_pix + w.e_lo + head, wpix.p + head, (size_t)(len - head), cudaMemcpyDeviceToHost, st));
-            GR_CUDA(cudaStreamSynchronize(st));
         }
+        GR_CUDA(cudaStreamSynchronize(pipe.cs));
+        GR_CUDA(cudaStreamSynchronize(st));
     }
     if (g->ooc) {
         int32_t h[32];

@@ -24,7 +24,8 @@ namespace {
 // ---- per-cell layout: sorted forward stencil, segment offsets, row length ----------------------------------
 __global__ void k_cell_fwd(int64_t ncell, int ncx, int ncy, int ncz, int periodic, const int32_t *__restrict__ cell_start,
                            int32_t *__restrict__ fwd_cell, int32_t *__restrict__ fwd_off, int32_t *__restrict__ nf,
-                           int32_t *__restrict__ rowlen, int64_t *__restrict__ rowbytes, int32_t *__restrict__ stats)
+                           int32_t *__restrict__ rowlen, int64_t *__restrict__ rowbytes, int32_t *__restrict__ stats,
+                           const uint8_t *__restrict__ keep)
 {
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncell) return;
@@ -63,10 +64,12 @@ __global__ void k_cell_fwd(int64_t ncell, int ncx, int ncy, int ncz, int periodi
         }
     }
     const int occ = cell_start[c + 1] - cell_start[c];
-    const int rl = (off + 31) & ~31;         // rows start on 32-byte sectors; row addresses fit 32 bits after >> 5
+    // rows start on 32-byte sectors (row addresses fit 32 bits after >> 5) and end with at least ONE pad byte, which
+    // stays 0xFF: the gather kernel points entries that have no segment in a row at it instead of predicating the load
+    const int rl = (off + 32) & ~31;
     nf[c] = m;
     rowlen[c] = rl;
-    rowbytes[c] = (int64_t)occ * rl;
+    rowbytes[c] = (keep && !keep[c]) ? 0 : (int64_t)occ * rl;      // slab graphs: no dense rows outside slab + halo
     if (occ > 0) {
         atomicMax(&stats[0], occ);
         atomicMax(&stats[1], rl);
@@ -194,7 +197,8 @@ bool gr_dense_tables(gramsci_graph *g)
     stats.alloc(2);
     GR_CUDA(cudaMemsetAsync(stats.p, 0, 8, st));
     k_cell_fwd<<<blocks_for(nc, 128), 128, 0, st>>>(nc, g->nc[0], g->nc[1], g->nc[2], g->periodic, g->cell_start.p,
-                                                    d.fwd_cell.p, d.fwd_off.p, d.nf.p, d.rowlen.p, rowbytes.p, stats.p);
+                                                    d.fwd_cell.p, d.fwd_off.p, d.nf.p, d.rowlen.p, rowbytes.p, stats.p,
+                                                    g->cell_keep.p);
     GR_CUDA(cudaGetLastError());
     gr_exclusive_scan<int64_t, int64_t>(rowbytes.p, nc, d.dbase.p, st);
     int32_t h[2];

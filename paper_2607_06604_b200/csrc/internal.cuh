@@ -82,6 +82,11 @@ struct GrWindow {
     int32_t row_lo = 0, row_hi = 0;   // rows [row_lo,row_hi)
     int64_t e_lo = 0, e_hi = 0;       // edges [e_lo,e_hi), e_lo rounded down to a multiple of 16
     int64_t d_lo = 0, d_hi = 0;       // dense cell-block rows of these rows: bytes [d_lo,d_hi) (spatial graphs)
+    // out-of-core: the window's edge arrays in ONE page-locked host block [idx | bin | pix]; entry 0 = edge e_lo
+    void *h_block = nullptr;
+    size_t h_block_bytes = 0;
+    int32_t *h_idx = nullptr;
+    uint8_t *h_bin = nullptr, *h_pix = nullptr;
 };
 
 // hub filter of the enumeration kernels (hub_stride: sampled partial result; shard_*: one shard of a multi-GPU run)
@@ -124,6 +129,9 @@ struct gramsci_graph {
     double r_min = 0, r_max = 0;
     double q[GR_MAXBINS + 1];      // squared bin edges (A-3)
     int weighted = 0, has_pix = 0, spatial = 0, algo = 0, hub_stride = 1, shard_count = 1, shard_index = 0;
+    int slab_count = 1, slab_index = 0;      // slab + halo partition (gramsci_options.slab_count)
+    int32_t hub_lo = 0, hub_hi = INT32_MAX;  // hubs this graph owns (internal labels); everything unless slab_count > 1
+    DevBuf<uint8_t> cell_keep;               // slab graphs: [ncell] 1 = rows of this cell are stored
     int algo_g = 0;                // gather kernel: forced warps per hub (test knob GRAMSCI_GATHER_G), 0 = choose
     double w_absmin = 1.0, w_absmax = 1.0;   // range of |w| (1 for unit weights): picks fixed-point or fp64 weighted sums
     cudaStream_t stream = nullptr;
@@ -162,9 +170,7 @@ struct gramsci_graph {
     int ooc = 0;
     std::vector<GrWindow> windows;
     std::vector<uint8_t> need;     // [W*W] need[h*W+c] = 1 iff some edge (i,j) has i in window h, j in window c
-    int32_t *h_idx = nullptr;      // pinned [E]
-    uint8_t *h_bin = nullptr, *h_pix = nullptr;
-    size_t h_idx_bytes = 0, h_bin_bytes = 0, h_pix_bytes = 0;
+    // (the pinned host arrays hang off the windows: GrWindow::h_block)
     // timing of the last calls
     double t_build_ms = 0, t_query_ms = 0, t_enum_ms = 0, n_launches = 0, staged_bytes = 0;
 };
@@ -181,8 +187,14 @@ int gr_kernel_occupancy(const void *fn, int threads, size_t smem);
 
 // page-locked host memory for the out-of-core windows (api.cu): anonymous mapping, pages touched by all
 // host cores, then cudaHostRegister -- cudaHostAlloc pins at 2.6 GiB/s on this box, this path at ~25 GiB/s
-void *gr_pinned_alloc(size_t bytes);
+// Freed blocks go to a process-wide cache (like the device pool, so that the next capped build does not pin 42 GB
+// again); gramsci_release_memory() unpins and unmaps them.  gr_pinned_alloc_nothrow is for the build's background
+// pinning thread (error text returned instead of the thread-local error state); `*bytes` is rounded up to the block
+// actually handed out, which is what gr_pinned_free takes back.
+void *gr_pinned_alloc_nothrow(size_t *bytes, std::string *err);
+void *gr_pinned_alloc(size_t *bytes);
 void gr_pinned_free(void *p, size_t bytes);
+void gr_pinned_release_cache();
 
 // ---- build_graph.cu -----------------------------------------------------------------------------
 void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights, int n_windows_forced);
@@ -198,8 +210,13 @@ struct GrView {
     const int64_t *ptr;
     const int32_t *idx_h; const uint8_t *bin_h; const uint8_t *pix_h; int64_t e0_h;
     const int32_t *idx_c; const uint8_t *bin_c; const uint8_t *pix_c; int64_t e0_c;
-    int32_t h_lo, h_hi;     // hub rows of this tile (labels)
+    int32_t h_lo, h_hi;     // hub rows of this tile (labels), already cut to the hubs the graph owns (slab graphs)
+    int32_t win_h;          // index of the hub window of this tile (0 in-core)
     int32_t c_lo, c_hi;     // resident search rows (labels)
+    // 4pCF under a memory cap: a SECOND resident search window; a tile (h, c1 <= c2) takes the tetrahedra
+    // (i, j1, j2, j3) with i in h, j1 in [c_lo,c_hi) and j2 in [c2_lo,c2_hi).  In-core: the same arrays as idx_c.
+    const int32_t *idx_c2; const uint8_t *bin_c2; int64_t e0_c2;
+    int32_t c2_lo, c2_hi;
     const int32_t *order;   // hub schedule (labels in spatial order), [n]
     int32_t s_lo, s_hi;     // schedule slots to walk (in-core: [0,n))
     const double *w;        // weights by label or nullptr
@@ -236,7 +253,9 @@ void gr_exclusive_scan(const InT *d_in, int64_t n, OutT *d_out, cudaStream_t st)
 struct GrTileRunner;
 typedef void (*gr_tile_fn)(gramsci_graph *g, const GrView &v, void *user, cudaStream_t st);
 // hub_only: visit each hub window once with no search window (2pCF sweep, work counters)
-void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense = false);
+// pair_search: tiles are (hub window h, search windows c1 <= c2) -- the 4pCF tiling of P:159 (three resident windows)
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense = false,
+                      bool pair_search = false);
 int gr_tiler_slots(const gramsci_graph *g, bool need_pix, bool need_dense);
 
 // host helpers (canon.cpp part of api.cu)

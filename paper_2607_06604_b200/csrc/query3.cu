@@ -817,7 +817,7 @@ void gr_3pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int equilater
     if (g->algo == GRAMSCI_ALGO_DEFAULT || g->algo == GRAMSCI_ALGO_GATHER) {
         const char *why = "";
         const size_t planes = (size_t)((!d_wsum || d_counts) ? 1 : 0) + (d_wsum ? 3 : 0);
-        const size_t hist_bytes = planes * (size_t)((nh + 31) & ~31) * 4;
+        const size_t hist_bytes = planes * (size_t)((nh + 32) & ~31) * 4;
         if (gr_gather_applicable(g, d_wsum != nullptr, hist_bytes, &why)) {
             gr_3pcf_gather(g, d_counts, d_wsum, equilateral);
             g->t_query_ms = total.stop();          // includes the one-off expansion of the dense rows

@@ -99,6 +99,14 @@ __device__ __forceinline__ double lds_f64(unsigned a)
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
     return v;
 }
+// one byte of a dense row through the read-only path, zero-extended into a 32-bit register (opaque to the compiler, which
+// otherwise re-masks the byte before every use)
+__device__ __forceinline__ unsigned ldg_u8(const uint8_t *p)
+{
+    unsigned v;
+    asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ unsigned sexch0(unsigned a)
 {
     unsigned v;
@@ -111,6 +119,20 @@ __device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned r
 {
     if (EQ) asm volatile("{\n .reg .pred q;\n setp.eq.u32 q, %1, %2;\n @q red.shared.add.u32 [%0], 1;\n}" ::"r"(a), "r"(bv), "r"(ref));
     else asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %1, 255;\n @q red.shared.add.u32 [%0], 1;\n}" ::"r"(a), "r"(bv));
+}
+// Branch-free form: a miss adds to a spare word behind the histogram (index nh; the drains never read it).  The
+// predicated form above compiles to BSSY / BRA / ATOMS.POPC.INC / BSYNC; this one to SEL / ATOMS.POPC.INC, and the lanes
+// of a warp that miss share one address, which the instruction aggregates.
+#ifndef G3_DUMMY_BIN
+#define G3_DUMMY_BIN 0
+#endif
+#ifndef G3_SPU
+#define G3_SPU 1
+#endif
+__device__ __forceinline__ void sred_inc_sel(unsigned a, unsigned bv, unsigned a_dummy)
+{
+    asm volatile("{\n .reg .pred q;\n .reg .u32 a2;\n setp.ne.u32 q, %1, 255;\n selp.u32 a2, %0, %2, q;\n red.shared.add.u32 [a2], 1;\n}"
+                 ::"r"(a), "r"(bv), "r"(a_dummy));
 }
 template <bool EQ>
 __device__ __forceinline__ void sred_limbs_hit(unsigned a, unsigned stride, unsigned l0, unsigned l1, unsigned l2, unsigned bv,
@@ -402,7 +424,14 @@ __device__ __forceinline__ void build_T_row32(const G3Tables &tb, int cj, int fc
     Trow[lane] = val;
 }
 
-template <int WMODE, bool EQ, bool OOC>
+// KMAJOR: the LANES keep their tail entries k in registers (a chunk of 128 per warp: position, ordinal, bin and, weighted,
+// w_k) and the loop runs over the SPOKES of a block of 32; what depends on the spoke alone (dense row, histogram plane,
+// w_i w_j) is warp-uniform, and the table offsets T[o_j][o_k] of the lane's four entries are reloaded only when the
+// spoke's cell changes (spokes are in label = cell order: every ~1/14 of a row).  Per 128 wedges that leaves ONE
+// shared-memory load next to the four byte gathers and the four histogram updates, instead of eight -- the kernel runs at
+// the LSU wavefront rate (profiles/r2_gather_cta_cfg5e.md), so loads are what is worth removing.  Work items (chunk,
+// spoke block) are dealt to the warps through a shared-memory counter.
+template <int WMODE, bool EQ, bool OOC, bool KMAJOR>
 __global__ void __launch_bounds__(G3_THREADS)
 k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restrict__ unit_counter,
                   unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
@@ -422,6 +451,8 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
     double *aw = (double *)(f_dbase + 32);
     uint32_t *kx = (uint32_t *)(aw + (WMODE ? p.row_cap : 0));
     __shared__ int f_occ[32];
+    __shared__ int s_item;                    // KMAJOR: next work item of the current unit
+    __shared__ int s_cum[514];                // KMAJOR: items before chunk c
     const unsigned a_hist = s_addr(hist), a_T = s_addr(T), a_kx = s_addr(kx), a_aw = s_addr(aw);
     const unsigned plane_b = (unsigned)p.nhp * 4;
     __shared__ int s_unit;
@@ -547,6 +578,129 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
             }
             __syncthreads();
             const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
+            if (KMAJOR) {
+                // chunk c = tail entries [t_base + 128 c, + 128); its spokes are [a_lo, min(a_hi, last entry of the chunk))
+                const int t_base = a_lo + 1;
+                const int n_chunks = (n - t_base + 127) >> 7;
+                if (threadIdx.x == 0) {
+                    int cum = 0;
+                    for (int c = 0; c < n_chunks; ++c) {
+                        s_cum[c] = cum;
+                        const int a_end = min(a_hi, min(n, t_base + 128 * c + 128) - 1);
+                        cum += (a_end - a_lo + 31) >> 5;
+                    }
+                    s_cum[n_chunks] = cum;
+                    s_item = 0;
+                }
+                __syncthreads();
+                const int n_items = s_cum[n_chunks];
+                int c = 0;
+                for (;;) {
+                    int item = 0;
+                    if (lane == 0) item = atomicAdd(&s_item, 1);
+                    item = __shfl_sync(0xffffffffu, item, 0);
+                    if (item >= n_items) break;
+                    while (s_cum[c + 1] <= item) ++c;                  // items come in ascending order
+                    const int t0 = t_base + 128 * c;
+                    const int a_end = min(a_hi, min(n, t0 + 128) - 1);
+                    const int sa = a_lo + 32 * (item - s_cum[c]), sb = min(a_end, sa + 32);
+                    unsigned pos[4], okk[4], hk[4];
+                    int tq[4];
+                    double wk[4];
+                    // byte address of (first row of the spoke's cell) + (offset of the lane's entry in such a row); null for an
+                    // entry whose cell is not forward of the spoke's (about half of the wedges: no load is issued for them --
+                    // pointing them at the 0xFF pad byte of the row instead costs more in sectors than the predicate does
+                    // in issue slots: cfg5 1/8 replica 2.04 s against 1.91 s)
+                    const uint8_t *pq[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        tq[q] = t0 + 32 * q + lane;
+                        const unsigned kk = (tq[q] < n) ? lds_u32(a_kx + 4u * tq[q]) : (31u << 16);
+                        pos[q] = kk & 0xffffu;
+                        okk[q] = (kk >> 14) & 0x7cu;
+                        hk[q] = EQ ? (kk >> 21) : (kk >> 21) * nb4;
+                        pq[q] = nullptr;
+                        if (WMODE) wk[q] = (tq[q] < n) ? lds_f64(a_aw + 8u * tq[q]) : 0.0;
+                    }
+                    int cur_oj = -1;
+                    unsigned rl5 = 0;                                  // row length of the spoke's cell in 32-byte sectors
+                    // one spoke: its four byte gathers (all issued before anything waits for them) ...
+                    auto gather = [&](int a, unsigned ea, auto TRIc, unsigned (&bv)[4]) {
+                        constexpr bool TRI = decltype(TRIc)::value;
+                        const unsigned rs = (ea & 0xffffu) * rl5;      // row of the spoke, in sectors from its cell's first row
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            bool act = pq[q] != nullptr;
+                            if (TRI) act = act && tq[q] > a;
+                            if (EQ) act = act && hk[q] == (ea >> 21);
+                            bv[q] = 0xffu;
+                            if (act) bv[q] = ldg_u8(pq[q] + (size_t)rs * 32u);
+                        }
+                    };
+                    // ... and its four histogram updates
+                    auto update = [&](int a, unsigned ea, const unsigned (&bv)[4]) {
+                        const unsigned ba = ea >> 21;
+                        const unsigned a_hj = EQ ? a_hist + ba * 4u : a_hist + ba * nb24;
+                        const double wia = WMODE ? wi * lds_f64(a_aw + 8u * a) : 0.0;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const unsigned ah = EQ ? a_hj : a_hj + hk[q] + bv[q] * 4u;
+                            if (have_cnt) {
+                                if (G3_DUMMY_BIN && !EQ) sred_inc_sel(ah, bv[q], a_hist + 4u * (unsigned)p.nh);
+                                else sred_inc_hit<EQ>(ah, bv[q], ba);
+                            }
+                            if (WMODE == 1) {
+                                unsigned l0, l1, l2;
+                                limbs_of(wia * wk[q], l0, l1, l2);
+                                sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], ba);
+                            } else if (WMODE == 2) {
+                                if (EQ ? (bv[q] == ba) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], wia * wk[q]);
+                            }
+                        }
+                    };
+                    auto spoke_loop = [&](int a_from, int a_to, auto TRIc) {
+                        for (int a = a_from; a < a_to;) {
+                            const unsigned ea = lds_u32(a_kx + 4u * a);
+                            const int oj = (ea >> 16) & 31;
+                            if (oj != cur_oj) {                        // warp-uniform: the spoke's cell changed
+                                cur_oj = oj;
+                                const unsigned a_Tj = a_T + (unsigned)oj * 128u;
+                                const uint8_t *cell_rows = v.dense + (f_dbase[oj] - v.d0);
+                                rl5 = (unsigned)f_rowlen[oj] >> 5;
+#pragma unroll
+                                for (int q = 0; q < 4; ++q) {
+                                    const unsigned o2 = lds_u32(a_Tj + okk[q]);
+                                    pq[q] = (o2 == ROW_NONE) ? nullptr : cell_rows + (o2 + pos[q]);
+                                }
+                            }
+                            unsigned bv[4];
+                            gather(a, ea, TRIc, bv);
+                            // G3_SPU 2: the next spoke's gathers are issued too when it lies in the same cell (eight loads in flight)
+                            unsigned ea2 = 0;
+                            bool two = false;
+                            if (G3_SPU == 2 && a + 1 < a_to) {
+                                ea2 = lds_u32(a_kx + 4u * (a + 1));
+                                two = (int)((ea2 >> 16) & 31) == oj;
+                            }
+                            if (two) {
+                                unsigned bv2[4];
+                                gather(a + 1, ea2, TRIc, bv2);
+                                update(a, ea, bv);
+                                update(a + 1, ea2, bv2);
+                                a += 2;
+                            } else {
+                                update(a, ea, bv);
+                                a += 1;
+                            }
+                        }
+                    };
+                    // spokes below every entry of the chunk need no t > a test
+                    const int s_mid = min(sb, max(sa, t0));
+                    spoke_loop(sa, s_mid, std::false_type());
+                    spoke_loop(s_mid, sb, std::true_type());
+                }
+                continue;                                              // next unit (the loop head synchronises)
+            }
             unsigned long long hbud = 0;          // WMODE 1: wedges of this hub since the last drain (rows beyond 724 entries)
             for (int a0 = a_lo; a0 < a_hi; a0 += G3_WARPS) {
                 if (WMODE == 1 && wedges > p.wflush) {
@@ -629,7 +783,8 @@ struct G3Run {
 template <int WMODE, bool EQ>
 gather_kernel_t gather_fn2(int cta, int ooc)
 {
-    if (cta) return ooc ? k_3pcf_gather_cta<WMODE, EQ, true> : k_3pcf_gather_cta<WMODE, EQ, false>;
+    if (cta == 2) return ooc ? k_3pcf_gather_cta<WMODE, EQ, true, true> : k_3pcf_gather_cta<WMODE, EQ, false, true>;
+    if (cta) return ooc ? k_3pcf_gather_cta<WMODE, EQ, true, false> : k_3pcf_gather_cta<WMODE, EQ, false, false>;
     return ooc ? k_3pcf_gather_warp<WMODE, EQ, true> : k_3pcf_gather_warp<WMODE, EQ, false>;
 }
 
@@ -651,8 +806,7 @@ void tile_3pcf_gather(gramsci_graph *g, const GrView &v, void *user, cudaStream_
         long long u_begin = 0;
         p.u_end = r->cta ? r->p.n_tile_units : (long long)r->p.n_units;
         if (g->ooc && !r->h_ubeg.empty()) {
-            size_t w = 0;
-            while (w + 1 < g->windows.size() && g->windows[w].row_lo != v.h_lo) ++w;
+            const size_t w = (size_t)v.win_h;
             u_begin = r->h_ubeg[w];
             p.u_end = r->h_uend[w];
         }
@@ -716,7 +870,7 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
     GrTimer total(st);
     const bool W = d_wsum != nullptr;
     G3Params p;
-    p.nb = nb; p.nh = nh; p.nhp = (nh + 31) & ~31;
+    p.nb = nb; p.nh = nh; p.nhp = (nh + 32) & ~31;      // at least one spare word behind the bins
     p.want_counts = d_counts ? 1 : 0;
     p.row_cap = std::max(16, (g->max_row + 15) & ~15);
     // weights: fp64 RED into per-CTA global slabs by default (measured faster than the limbs on every workload:
@@ -785,7 +939,11 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
         if (un.n == 0) continue;
         if (r.smem > g->smem_optin)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf (gather): histogram or longest row (%d entries) does not fit in shared memory", g->max_row);
-        r.fn = gather_fn(wmode, r.eq, k, g->ooc);
+        // long rows: lanes keep their tail entries, the loop runs over the spokes (KMAJOR); GRAMSCI_CTA_KMAJOR=0 selects the
+        // spoke-per-warp loop (kept for the ablation); the limb path (WMODE 1) needs its mid-hub drains and stays there
+        int kmajor = (wmode != 1 && g->max_row <= 65000) ? 1 : 0;
+        if (const char *e = getenv("GRAMSCI_CTA_KMAJOR")) kmajor = kmajor && atoi(e) != 0;
+        r.fn = gather_fn(wmode, r.eq, (k && kmajor) ? 2 : k, g->ooc);
         if (const char *e = getenv("GRAMSCI_CARVEOUT"))      // experiment: shared-memory carve-out in percent (L1 gets the rest)
             cudaFuncSetAttribute((const void *)r.fn, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(e));
         int occ = gr_kernel_occupancy((const void *)r.fn, G3_THREADS, r.smem);

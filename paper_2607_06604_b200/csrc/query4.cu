@@ -47,6 +47,7 @@ struct Q4Params {
     int n_shards;
     int ncfg;            // LUT path: number of canonical configurations (histograms are indexed by configuration)
     unsigned long long flush;   // LUT path: a warp drains the CTA histograms before its hit budget passes this
+    int ooc;             // capped graph: tile (h, c1 <= c2) of P:159 -- spoke rows come from two resident search windows
 };
 
 __constant__ int8_t c_perm4[24][4] = {
@@ -128,6 +129,7 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         if (s >= v.s_hi) break;
         const int32_t i = v.order[s];
         if (!GR_HUB_SELECTED(v, i)) continue;
+        if (i < v.h_lo || i >= v.h_hi) continue;               // hub of another window (capped graphs)
         const int64_t rb = v.ptr[i], re = v.ptr[i + 1];
         const int n = (int)(re - rb);
         if (n < 3) continue;                                   // a 4-clique needs three spokes
@@ -159,6 +161,15 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
             const int nj = (int)(je - jb);
             const int32_t *B = v.idx_c + (jb - v.e0_c);
             const uint8_t *Bb = v.bin_c + (jb - v.e0_c);
+            if (p.ooc) {
+                // rows of j1 come from search window c1, rows of j2 from c2; other rows are not resident and
+                // not needed: this tile only follows local edges (a, b) with k_a in c1 and k_b in c2
+                if (j >= v.c_lo && j < v.c_hi) {
+                } else if (j >= v.c2_lo && j < v.c2_hi) {
+                    B = v.idx_c2 + (jb - v.e0_c2);
+                    Bb = v.bin_c2 + (jb - v.e0_c2);
+                } else continue;
+            }
             const int32_t t_last = a_idx[n - 1];
             uint8_t *Da = D + (size_t)a * ld;
             uint32_t *Ba = bits + (size_t)a * nw;
@@ -252,9 +263,11 @@ k_4pcf(GrView v, Q4Params p, unsigned int *__restrict__ hub_counter, uint8_t *sc
         int qn = 0;                                            // warp-uniform queue fill
         for (int a = warp; a < n - 2; a += Q4_WARPS) {
             const uint32_t *Ba = bits + (size_t)a * nw;
+            if (p.ooc && (a_idx[a] < v.c_lo || a_idx[a] >= v.c_hi)) continue;      // j1 belongs to another tile
             for (int w = (a + 1) >> 5; w < nw; ++w) {          // lanes scan the 32 candidates b of word w
                 const int bcand = (w << 5) + lane;
-                const bool edge = bcand > a && bcand < n - 1 && ((Ba[w] >> lane) & 1u);
+                bool edge = bcand > a && bcand < n - 1 && ((Ba[w] >> lane) & 1u);
+                if (p.ooc && edge) edge = a_idx[bcand] >= v.c2_lo && a_idx[bcand] < v.c2_hi;   // j2 in window c2
                 const unsigned m = __ballot_sync(0xffffffffu, edge);
                 if (edge) my_q[qn + __popc(m & lt_mask)] = ((uint32_t)a << 16) | (uint32_t)bcand;
                 qn += __popc(m);
@@ -436,7 +449,6 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
 {
     cudaStream_t st = g->stream;
     const int nb = g->nb;
-    if (g->ooc) GR_FAIL(GRAMSCI_EINVAL, "4pcf: out-of-core graphs are not supported (build without device_mem_cap_bytes)");
     int64_t nh = 1;
     for (int e = 0; e < 6; ++e) nh *= nb;
     GrTimer total(st);
@@ -450,6 +462,7 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
     p.want_counts = (d_even_c || d_odd_c) ? 1 : 0;
     p.row_cap = std::max(16, (g->max_row + 15) & ~15);
     p.flush = gr_flush_budget(1ull << 27);
+    p.ooc = g->ooc ? 1 : 0;
     const int channels = (d_even_c ? 1 : 0) + (d_odd_c ? 1 : 0) + (d_even_w ? 1 : 0) + (d_odd_w ? 1 : 0);
     if (channels == 0) { GR_CUDA(cudaStreamSynchronize(st)); g->t_query_ms = total.stop(); return; }
     {   // raw histograms kept per launch: counts and/or weights, three sign classes each for the parity split
@@ -536,28 +549,30 @@ void gr_4pcf(gramsci_graph *g, int parity, uint64_t *d_even_c, int64_t *d_odd_c,
         GR_CUDA(cudaStreamSynchronize(st));      // h goes out of scope
     }
 
-    GrView v;
-    v.ptr = g->ptr.p; v.order = g->order.p; v.w = g->w.p; v.hub_stride = g->hub_stride; v.shard_count = g->shard_count; v.shard_index = g->shard_index;
-    v.idx_h = v.idx_c = g->idx.p; v.bin_h = v.bin_c = g->bin.p;
-    v.pix_h = v.pix_c = g->has_pix ? g->pix.p : nullptr;
-    v.e0_h = v.e0_c = 0;
-    v.h_lo = v.c_lo = 0; v.h_hi = v.c_hi = (int32_t)g->n;
-    v.s_lo = 0; v.s_hi = (int32_t)g->n;
+    struct Run {
+        Q4Params p; bool small, use_lut; int grid; size_t smem, stride;
+        unsigned int *counter; uint8_t *scratch; const double *tab; const uint32_t *lut;
+        unsigned long long *ce, *co; double *we, *wo;
+    } run{p, small, use_lut, grid, smem, stride, counter.p, scratch.p, tab.p, g->lut4.p, ce.p, co.p,
+          (d_even_w || d_odd_w) ? we.p : nullptr, wo.p};
+    // one launch per tile: the whole graph in-core; (hub window, search windows c1 <= c2) under a memory cap
+    auto tile_fn = [](gramsci_graph *gg, const GrView &v, void *user, cudaStream_t s) {
+        Run &r = *(Run *)user;
+        GR_CUDA(cudaMemsetAsync(r.counter, 0, sizeof(unsigned int), s));
+        if (r.small && r.use_lut)
+            k_4pcf<true, true><<<r.grid, Q4_THREADS, r.smem, s>>>(v, r.p, r.counter, r.scratch, r.stride, r.tab, r.lut, r.ce, r.co, r.we, r.wo);
+        else if (r.small)
+            k_4pcf<true, false><<<r.grid, Q4_THREADS, r.smem, s>>>(v, r.p, r.counter, r.scratch, r.stride, r.tab, nullptr, r.ce, r.co, r.we, r.wo);
+        else if (r.use_lut)
+            k_4pcf<false, true><<<r.grid, Q4_THREADS, r.smem, s>>>(v, r.p, r.counter, r.scratch, r.stride, r.tab, r.lut, r.ce, r.co, r.we, r.wo);
+        else
+            k_4pcf<false, false><<<r.grid, Q4_THREADS, r.smem, s>>>(v, r.p, r.counter, r.scratch, r.stride, r.tab, nullptr, r.ce, r.co, r.we, r.wo);
+        GR_CUDA(cudaGetLastError());
+        gg->n_launches += 1;
+    };
     {
         GrTimer en(st);
-        if (g->n > 0) {
-            double *wep = (d_even_w || d_odd_w) ? we.p : nullptr;
-            if (small && use_lut)
-                k_4pcf<true, true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, g->lut4.p, ce.p, co.p, wep, wo.p);
-            else if (small)
-                k_4pcf<true, false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, nullptr, ce.p, co.p, wep, wo.p);
-            else if (use_lut)
-                k_4pcf<false, true><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, g->lut4.p, ce.p, co.p, wep, wo.p);
-            else
-                k_4pcf<false, false><<<grid, Q4_THREADS, smem, st>>>(v, p, counter.p, scratch.p, stride, tab.p, nullptr, ce.p, co.p, wep, wo.p);
-            GR_CUDA(cudaGetLastError());
-            g->n_launches += 1;
-        }
+        if (g->n > 0) gr_for_each_tile(g, p.parity != 0, false, tile_fn, &run, false, true);
         g->t_enum_ms = en.stop();
     }
     if (use_lut) {

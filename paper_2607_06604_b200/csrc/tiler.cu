@@ -37,7 +37,7 @@ int gr_tiler_slots(const gramsci_graph *g, bool need_pix, bool need_dense)
     return std::min(K, 8);
 }
 
-void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense)
+void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn fn, void *user, bool need_dense, bool pair_search)
 {
     cudaStream_t st = g->stream;
     GrView v;
@@ -54,11 +54,16 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         v.bin_h = v.bin_c = g->bin.p;
         v.pix_h = v.pix_c = g->has_pix ? g->pix.p : nullptr;
         v.e0_h = v.e0_c = 0;
-        v.h_lo = v.c_lo = 0;
-        v.h_hi = v.c_hi = (int32_t)g->n;
-        v.s_lo = 0;
-        v.s_hi = (int32_t)g->n;
-        fn(g, v, user, st);
+        v.c_lo = 0;
+        v.c_hi = (int32_t)g->n;
+        v.h_lo = std::max(0, g->hub_lo);
+        v.h_hi = (int32_t)std::min<int64_t>(g->n, g->hub_hi);
+        v.win_h = 0;
+        v.idx_c2 = v.idx_c; v.bin_c2 = v.bin_c; v.e0_c2 = 0;
+        v.c2_lo = 0; v.c2_hi = (int32_t)g->n;
+        v.s_lo = g->spatial ? v.h_lo : 0;
+        v.s_hi = g->spatial ? v.h_hi : (int32_t)g->n;
+        if (v.h_hi > v.h_lo) fn(g, v, user, st);
         return;
     }
 
@@ -68,6 +73,8 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     for (auto &w : g->windows) { maxlen = std::max(maxlen, w.e_hi - w.e_lo); maxdense = std::max(maxdense, w.d_hi - w.d_lo); }
     if (!need_dense) maxdense = 0;
     const int K = gr_tiler_slots(g, need_pix, need_dense);
+    if (pair_search && K < 3)
+        GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for three windows of %lld edges (4pCF tiles, P:159)", (long long)maxlen);
     if (K < (hub_only ? 1 : 2)) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for two windows of %lld edges", (long long)maxlen);
 
     std::vector<Slot> slots(K);
@@ -126,10 +133,10 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         const int64_t len = w.e_hi - w.e_lo;
         if (s.wid >= 0) GR_CUDA(cudaStreamWaitEvent(cs, s.done, 0));     // last kernel reading it has finished
         if (len > 0) {
-            GR_CUDA(cudaMemcpyAsync(s.idx.p, g->h_idx + w.e_lo, (size_t)len * 4, cudaMemcpyHostToDevice, cs));
-            GR_CUDA(cudaMemcpyAsync(s.bin.p, g->h_bin + w.e_lo, (size_t)len, cudaMemcpyHostToDevice, cs));
+            GR_CUDA(cudaMemcpyAsync(s.idx.p, w.h_idx, (size_t)len * 4, cudaMemcpyHostToDevice, cs));
+            GR_CUDA(cudaMemcpyAsync(s.bin.p, w.h_bin, (size_t)len, cudaMemcpyHostToDevice, cs));
             if (g->has_pix && need_pix)
-                GR_CUDA(cudaMemcpyAsync(s.pix.p, g->h_pix + w.e_lo, (size_t)len, cudaMemcpyHostToDevice, cs));
+                GR_CUDA(cudaMemcpyAsync(s.pix.p, w.h_pix, (size_t)len, cudaMemcpyHostToDevice, cs));
             g->staged_bytes += (double)len * (5 + ((g->has_pix && need_pix) ? 1 : 0));
         }
         GR_CUDA(cudaEventRecord(s.ready, cs));
@@ -139,36 +146,54 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         return victim;
     };
 
-    std::vector<std::pair<int, int>> tiles;
+    // tiles (h, c1, c2): 2pCF / 3pCF use c2 == c1; the 4pCF takes every pair c1 <= c2 of search windows the hub window
+    // reaches (and, for c1 < c2, only if window c1 holds an edge into window c2 -- j1 ~ j2 is part of every tetrahedron)
+    struct Tile { int h, c1, c2; };
+    std::vector<Tile> tiles;
+    auto needed = [&](int h, int c) { return g->need.empty() || g->need[(size_t)h * W + c]; };
     for (int h = 0; h < W; ++h) {
-        if (hub_only) { tiles.push_back({h, h}); continue; }
-        for (int c = 0; c < W; ++c)
-            if (g->need.empty() || g->need[(size_t)h * W + c]) tiles.push_back({h, c});
+        if (std::min(g->windows[h].row_hi, g->hub_hi) <= std::max(g->windows[h].row_lo, g->hub_lo) && W > 1) continue;   // no owned hub
+        if (hub_only) { tiles.push_back({h, h, h}); continue; }
+        for (int c = 0; c < W; ++c) {
+            if (!needed(h, c)) continue;
+            if (!pair_search) { tiles.push_back({h, c, c}); continue; }
+            for (int c2 = c; c2 < W; ++c2)
+                if (needed(h, c2) && (c2 == c || needed(c, c2))) tiles.push_back({h, c, c2});
+        }
     }
     const int T = (int)tiles.size();
     for (int t = 0; t < T; ++t) {
-        const int a = acquire(tiles[t].first, 0);
-        const int b = acquire(tiles[t].second, 1u << a, need_dense);
-        if (a < 0 || b < 0) GR_FAIL(GRAMSCI_ENOMEM, "window cache exhausted");
+        const int a = acquire(tiles[t].h, 0);
+        const int b = acquire(tiles[t].c1, 1u << a, need_dense);
+        const int c = acquire(tiles[t].c2, (1u << a) | (1u << b), false);
+        if (a < 0 || b < 0 || c < 0) GR_FAIL(GRAMSCI_ENOMEM, "window cache exhausted");
         GR_CUDA(cudaStreamWaitEvent(st, slots[a].ready, 0));
         GR_CUDA(cudaStreamWaitEvent(st, slots[b].ready, 0));
-        const GrWindow &wh = g->windows[tiles[t].first], &wc = g->windows[tiles[t].second];
+        GR_CUDA(cudaStreamWaitEvent(st, slots[c].ready, 0));
+        const GrWindow &wh = g->windows[tiles[t].h], &wc = g->windows[tiles[t].c1], &wc2 = g->windows[tiles[t].c2];
         v.idx_h = slots[a].idx.p; v.bin_h = slots[a].bin.p; v.pix_h = slots[a].pix.p; v.e0_h = wh.e_lo;
         v.idx_c = slots[b].idx.p; v.bin_c = slots[b].bin.p; v.pix_c = slots[b].pix.p; v.e0_c = wc.e_lo;
-        v.h_lo = wh.row_lo; v.h_hi = wh.row_hi;
+        v.idx_c2 = slots[c].idx.p; v.bin_c2 = slots[c].bin.p; v.e0_c2 = wc2.e_lo;
+        v.h_lo = std::max(wh.row_lo, g->hub_lo); v.h_hi = std::min(wh.row_hi, g->hub_hi);
+        v.win_h = tiles[t].h;
         v.c_lo = wc.row_lo; v.c_hi = wc.row_hi;
+        v.c2_lo = wc2.row_lo; v.c2_hi = wc2.row_hi;
         v.dense = need_dense ? slots[b].dense.p : nullptr;
         v.d0 = wc.d_lo;
-        if (g->spatial) { v.s_lo = wh.row_lo; v.s_hi = wh.row_hi; }
+        if (g->spatial) { v.s_lo = v.h_lo; v.s_hi = v.h_hi; }
         else { v.s_lo = 0; v.s_hi = (int32_t)g->n; }
-        fn(g, v, user, st);
+        if (v.h_hi > v.h_lo) fn(g, v, user, st);
         GR_CUDA(cudaEventRecord(slots[a].done, st));
         if (b != a) GR_CUDA(cudaEventRecord(slots[b].done, st));
+        if (c != a && c != b) GR_CUDA(cudaEventRecord(slots[c].done, st));
         // prefetch the next tile's windows into slots the running tile does not use (copy stream)
         if (t + 1 < T) {
-            unsigned protect = (1u << a) | (1u << b);
-            int s1 = acquire(tiles[t + 1].first, protect);
-            if (s1 >= 0) acquire(tiles[t + 1].second, protect | (1u << s1), need_dense);
+            unsigned protect = (1u << a) | (1u << b) | (1u << c);
+            int s1 = acquire(tiles[t + 1].h, protect);
+            if (s1 >= 0) {
+                int s2 = acquire(tiles[t + 1].c1, protect | (1u << s1), need_dense);
+                if (s2 >= 0 && tiles[t + 1].c2 != tiles[t + 1].c1) acquire(tiles[t + 1].c2, protect | (1u << s1) | (1u << s2), false);
+            }
         }
     }
     GR_CUDA(cudaStreamSynchronize(st));

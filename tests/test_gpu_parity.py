@@ -442,6 +442,31 @@ def test_3pcf_bao_replica(algo):
     assert np.array_equal(c, oc)
 
 
+@pytest.mark.parametrize("kmajor", ["1", "0"])
+def test_gather_cta_loop_orders(kmajor, monkeypatch):
+    """The long-row gather kernel in both loop orders (GRAMSCI_CTA_KMAJOR=1: lanes keep their tail entries and loop
+    over the spokes, the default; 0: one spoke per warp, tail streamed): counts, fp64 weighted sums and the
+    equilateral restriction against the oracle, with small spoke tiles and histogram drains forced."""
+    monkeypatch.setenv("GRAMSCI_CTA_KMAJOR", kmajor)
+    cfg, oc = _bao_replica()
+    for tile_mb, budget in (("", ""), ("1", "2500")):
+        if tile_mb:
+            monkeypatch.setenv("GRAMSCI_TILE_MB", tile_mb)
+            monkeypatch.setenv("GRAMSCI_FLUSH_BUDGET", budget)
+        gg = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], algo=gr.ALGO_GATHER)
+        assert gg.info()["max_row"] > 2000
+        assert np.array_equal(gg.pcf3()[0], oc)
+        assert np.array_equal(gg.pcf3_equilateral()[0], oc.reshape(18, 18, 18)[np.arange(18), np.arange(18), np.arange(18)])
+    c5 = cat.config5(seed=5102, n=3_000, L=310.0)
+    w = np.random.default_rng(9).uniform(0.5, 1.5, 3000)
+    og = oracle.Graph(c5["points"], w, c5["box"], c5["r_min"], c5["r_max"], c5["nbins"])
+    gw = gr.gramsci_build_graph(c5["points"], w, c5["box"], c5["r_min"], c5["r_max"], c5["nbins"], algo=gr.ALGO_GATHER)
+    c, ws = gw.pcf3(weighted=True)
+    o_c, o_w = og.pcf3()
+    assert gw.info()["max_row"] > 800 and np.array_equal(c, o_c)
+    assert_weighted_close(ws, o_w)
+
+
 @pytest.mark.parametrize("relabel", [1, 2])
 @pytest.mark.parametrize("n_windows,cap_frac", [(2, 1.2), (5, 1.0), (7, 0.45)])
 def test_out_of_core_equals_in_core(relabel, n_windows, cap_frac):
@@ -494,8 +519,44 @@ def test_out_of_core_cap_derives_windows():
     _, g1 = build_both(cfg, device_mem_cap_bytes=csr // 2)
     assert g1.info()["n_windows"] >= 8           # four window buffers must fit under the cap
     assert np.array_equal(g1.pcf3()[0], og.pcf3()[0])
-    with pytest.raises(gr.GramsciError):
-        g1.pcf4()
+    assert np.array_equal(g1.pcf4()[0], og.pcf4()[0])      # 4pCF tiles over (h, c1 <= c2)
+
+
+@pytest.mark.parametrize("relabel,n_windows", [(1, 3), (1, 6), (2, 4)])
+def test_out_of_core_4pcf_equals_in_core(relabel, n_windows):
+    """under a memory cap the 4pCF runs over tiles (hub window h, search windows c1 <= c2); every tetrahedron
+    lands in exactly one tile, so counts equal the resident run and the oracle bit for bit (C-13), weighted sums to
+    A-13's tolerance.  relabel=2 keeps caller labels (every window reaches every window)."""
+    cfg = small(35, n=5000, L=36.0, weighted=True, r_max=5.0, nb=4)
+    og, g0 = build_both(cfg, relabel=relabel)
+    oc, ow = og.pcf4()
+    csr = g0.info()["csr_bytes"]
+    _, g1 = build_both(cfg, relabel=relabel, device_mem_cap_bytes=int(csr * 2.0), n_windows=n_windows)
+    assert g1.info()["n_windows"] == n_windows
+    c, w = g1.pcf4(weighted=True)
+    assert c.sum() == oc.sum() > 0
+    assert np.array_equal(c, oc)
+    assert np.array_equal(c, g0.pcf4()[0])
+    assert_weighted_close(w, ow)
+    assert g1.timing(4) >= csr * 0.99
+
+
+@pytest.mark.parametrize("n_windows", [3, 5])
+def test_out_of_core_4pcf_parity_equals_in_core(n_windows):
+    """The parity-decomposed 4pCF (caller labels, pixel bytes staged with the hub window) under a cap: all four
+    channels against the oracle."""
+    c4 = cat.config4(seed=4005, n=4000, cap_deg=6.0)
+    o4 = oracle.Graph(c4["points"], c4["weights"], None, c4["r_min"], c4["r_max"], c4["nbins"])
+    rec, rew, roc, row = o4.pcf4(parity=True)
+    g0 = gr.gramsci_build_graph(c4["points"], c4["weights"], None, c4["r_min"], c4["r_max"], c4["nbins"], want_pixels=True)
+    csr = g0.info()["csr_bytes"]
+    g1 = gr.gramsci_build_graph(c4["points"], c4["weights"], None, c4["r_min"], c4["r_max"], c4["nbins"], want_pixels=True,
+                                device_mem_cap_bytes=int(csr * 2.0), n_windows=n_windows)
+    assert g1.info()["n_windows"] == n_windows
+    ec, oc, ew, ow = g1.pcf4_parity(weighted=True)
+    assert ec.sum() == rec.sum() > 0
+    assert np.array_equal(ec, rec) and np.array_equal(oc, roc)
+    assert np.all(np.abs(ew - rew) <= 1e-10 * np.abs(rew)) and np.all(np.abs(ow - row) <= 1e-10 * np.abs(rew))
 
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times ------------------------------------
@@ -720,6 +781,51 @@ def test_hub_shards_add_up_to_the_full_result():
         assert_weighted_close(gow, ow, scale=np.abs(ew))
     with pytest.raises(gr.GramsciError):
         gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], shard_count=2, shard_index=2)
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("algo", [0, 2, 3])
+def test_slab_and_halo_partition_adds_up(periodic, algo):
+    """S:8(e): one slab of cells per device, each holding only the rows of its slab and of the halo its
+    hubs' spokes live in.  The slabs own disjoint hub ranges covering the catalogue, every slab stores fewer edges
+    than the full graph, and the 2pCF / 3pCF / 4pCF histograms of the slabs sum to the oracle's (counts exactly) --
+    here the slabs run one after the other on one GPU; also under a memory cap (windows) per slab."""
+    cfg = small(53, n=12000, L=60.0, weighted=True, r_max=5.0, nb=5, periodic=periodic)
+    og = oracle.Graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"])
+    oc2, ow2 = og.pcf2()
+    oc3, ow3 = og.pcf3()
+    oc4, ow4 = og.pcf4()
+    n = cfg["points"].shape[0]
+    for world in (2, 5):
+        c2 = np.zeros_like(oc2); w2 = np.zeros_like(ow2); c3 = np.zeros_like(oc3); w3 = np.zeros_like(ow3)
+        c4 = np.zeros_like(oc4); w4 = np.zeros_like(ow4); cc3 = np.zeros_like(oc3)
+        cover, stored = [], []
+        for rank in range(world):
+            g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                       slab_count=world, slab_index=rank, algo=algo)
+            cover.append(g.slab_range())
+            stored.append(g.info()["n_edges"])
+            a, b = g.pcf2(weighted=True); c2 += a; w2 += b
+            a, b = g.pcf3(weighted=True); c3 += a; w3 += b
+            a, b = g.pcf4(weighted=True); c4 += a; w4 += b
+            csr = g.info()["csr_bytes"]
+            g.free()
+            gc = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
+                                        slab_count=world, slab_index=rank, algo=algo, device_mem_cap_bytes=max(csr, 4096) * 2,
+                                        n_windows=3)
+            cc3 += gc.pcf3()[0]
+            gc.free()
+        assert cover[0][0] == 0 and cover[-1][1] == n and all(cover[k][1] == cover[k + 1][0] for k in range(world - 1))
+        assert all(hi > lo for lo, hi in cover)                      # every slab got hubs (work-balanced cut)
+        assert max(stored) < og.n_edges and sum(stored) >= og.n_edges
+        if world == 5:
+            assert max(stored) < 0.6 * og.n_edges                    # slab + halo, not the whole graph
+        assert np.array_equal(c2, oc2) and np.array_equal(c3, oc3) and np.array_equal(c4, oc4) and np.array_equal(cc3, oc3)
+        assert_weighted_close(w2, ow2); assert_weighted_close(w3, ow3); assert_weighted_close(w4, ow4)
+    with pytest.raises(gr.GramsciError):                             # needs cell-order labels
+        gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], slab_count=2, relabel=2)
+    with pytest.raises(gr.GramsciError):
+        gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], slab_count=2, shard_count=2)
 
 
 def test_many_bins_global_histogram_path():
