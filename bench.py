@@ -185,6 +185,10 @@ def workload(name: str, seed_shift: int = 0):
     """List of catalogues (dicts from catalogues.py) making up one batch."""
     if name == "cfg2":
         return [cat.config2_data(seed=2001 + seed_shift), cat.config2_randoms(seed=2002 + seed_shift)]
+    if name == "cfg2r":       # the uniform randoms of configs[1] alone (unit weights): the ablation / profiling case
+        return [cat.config2_randoms(seed=2002 + seed_shift)]
+    if name == "cfg2d":       # the weighted clustered catalogue of configs[1] alone
+        return [cat.config2_data(seed=2001 + seed_shift)]
     if name == "cfg2small":   # 1/8 replica (same densities) for quick checks
         return [cat.config2_data(seed=2001 + seed_shift, n=125_000, L=500.0, mean_parents=1250.0),
                 cat.config2_randoms(seed=2002 + seed_shift, n=125_000, L=500.0)]

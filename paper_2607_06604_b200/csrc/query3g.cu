@@ -124,10 +124,10 @@ __device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned r
 // predicated form above compiles to BSSY / BRA / ATOMS.POPC.INC / BSYNC; this one to SEL / ATOMS.POPC.INC, and the lanes
 // of a warp that miss share one address, which the instruction aggregates.
 #ifndef G3_DUMMY_BIN
-#define G3_DUMMY_BIN 0
+#define G3_DUMMY_BIN 1
 #endif
 #ifndef G3_SPU
-#define G3_SPU 1
+#define G3_SPU 2
 #endif
 __device__ __forceinline__ void sred_inc_sel(unsigned a, unsigned bv, unsigned a_dummy)
 {
@@ -453,6 +453,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
     __shared__ int f_occ[32];
     __shared__ int s_item;                    // KMAJOR: next work item of the current unit
     __shared__ int s_cum[514];                // KMAJOR: items before chunk c
+    __shared__ int s_cf[34];                  // KMAJOR: first staged row entry whose cell ordinal is >= o (entries are in cell order)
     const unsigned a_hist = s_addr(hist), a_T = s_addr(T), a_kx = s_addr(kx), a_aw = s_addr(aw);
     const unsigned plane_b = (unsigned)p.nhp * 4;
     __shared__ int s_unit;
@@ -576,9 +577,16 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                 kx[t] = (unsigned)(k - f_start[ok]) | ((unsigned)ok << 16) | ((unsigned)gb[t] << 21);
                 if (WMODE) aw[t] = v.w[k];
             }
+            if (KMAJOR && threadIdx.x < 34) s_cf[threadIdx.x] = n;
             __syncthreads();
             const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
             if (KMAJOR) {
+                // runs of spokes of one cell: s_cf[o] = first entry with ordinal >= o (ordinals may skip empty cells)
+                for (int t = a_lo + threadIdx.x; t < n; t += G3_THREADS) {
+                    const int o = (int)((kx[t] >> 16) & 31u);
+                    const int op = (t > a_lo) ? (int)((kx[t - 1] >> 16) & 31u) : -1;
+                    for (int x = op + 1; x <= o; ++x) s_cf[x] = t;
+                }
                 // chunk c = tail entries [t_base + 128 c, + 128); its spokes are [a_lo, min(a_hi, last entry of the chunk))
                 const int t_base = a_lo + 1;
                 const int n_chunks = (n - t_base + 127) >> 7;
@@ -622,7 +630,6 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                         pq[q] = nullptr;
                         if (WMODE) wk[q] = (tq[q] < n) ? lds_f64(a_aw + 8u * tq[q]) : 0.0;
                     }
-                    int cur_oj = -1;
                     unsigned rl5 = 0;                                  // row length of the spoke's cell in 32-byte sectors
                     // one spoke: its four byte gathers (all issued before anything waits for them) ...
                     auto gather = [&](int a, unsigned ea, auto TRIc, unsigned (&bv)[4]) {
@@ -658,12 +665,16 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                             }
                         }
                     };
+                    // spokes [a_from, a_to): cell by cell (the table offsets of the lane's entries depend on the spoke's cell
+                    // only), G3_SPU spokes at a time with all their gathers issued before the first histogram update
                     auto spoke_loop = [&](int a_from, int a_to, auto TRIc) {
-                        for (int a = a_from; a < a_to;) {
-                            const unsigned ea = lds_u32(a_kx + 4u * a);
-                            const int oj = (ea >> 16) & 31;
-                            if (oj != cur_oj) {                        // warp-uniform: the spoke's cell changed
-                                cur_oj = oj;
+                        constexpr bool TRI = decltype(TRIc)::value;
+                        constexpr int SPU = TRI ? 1 : G3_SPU;
+                        int a = a_from;
+                        while (a < a_to) {
+                            const int oj = (int)((lds_u32(a_kx + 4u * a) >> 16) & 31u);
+                            const int run_end = min(a_to, s_cf[oj + 1]);
+                            {
                                 const unsigned a_Tj = a_T + (unsigned)oj * 128u;
                                 const uint8_t *cell_rows = v.dense + (f_dbase[oj] - v.d0);
                                 rl5 = (unsigned)f_rowlen[oj] >> 5;
@@ -673,24 +684,20 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                                     pq[q] = (o2 == ROW_NONE) ? nullptr : cell_rows + (o2 + pos[q]);
                                 }
                             }
-                            unsigned bv[4];
-                            gather(a, ea, TRIc, bv);
-                            // G3_SPU 2: the next spoke's gathers are issued too when it lies in the same cell (eight loads in flight)
-                            unsigned ea2 = 0;
-                            bool two = false;
-                            if (G3_SPU == 2 && a + 1 < a_to) {
-                                ea2 = lds_u32(a_kx + 4u * (a + 1));
-                                two = (int)((ea2 >> 16) & 31) == oj;
+                            for (; a + SPU <= run_end; a += SPU) {
+                                unsigned ea[SPU], bv[SPU][4];
+#pragma unroll
+                                for (int u = 0; u < SPU; ++u) ea[u] = lds_u32(a_kx + 4u * (a + u));
+#pragma unroll
+                                for (int u = 0; u < SPU; ++u) gather(a + u, ea[u], TRIc, bv[u]);
+#pragma unroll
+                                for (int u = 0; u < SPU; ++u) update(a + u, ea[u], bv[u]);
                             }
-                            if (two) {
-                                unsigned bv2[4];
-                                gather(a + 1, ea2, TRIc, bv2);
+                            for (; a < run_end; ++a) {
+                                const unsigned ea = lds_u32(a_kx + 4u * a);
+                                unsigned bv[4];
+                                gather(a, ea, TRIc, bv);
                                 update(a, ea, bv);
-                                update(a + 1, ea2, bv2);
-                                a += 2;
-                            } else {
-                                update(a, ea, bv);
-                                a += 1;
                             }
                         }
                     };
