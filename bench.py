@@ -435,13 +435,14 @@ def roofline_3pcf(name, w, launch_ms, hbm, hbm_kind, peaks):
                         "catalogues: hits/s over these measured rates is the atomic-path utilisation"}}
 
 
-def roofline_4pcf(w, launch_ms, channels, peaks):
+def roofline_4pcf(name, w, launch_ms, channels, peaks):
     """4pCF kernels: one global RED per hit and kind of output into nb^6 raw bins; the bound is the
     global atomic rate, measured in this run."""
     rate = w["hits"] * channels / (launch_ms * 1e-3) / 1e9
     peak = peaks["red_u64_gops"] if channels == 1 else min(peaks["red_u64_gops"], peaks["red_f64_gops"])
-    return {"bound": "l2-atomics", "achieved": rate, "peak": peak, "unit": "Gatomic/s", "frac": rate / peak, "traffic": None,
-            "kernel": f"k_4pcf on {w['name']}", "launch_ms": launch_ms,
+    traffic, src = dram_traffic(f"{name}:{w['name']}")
+    return {"bound": "l2-atomics", "achieved": rate, "peak": peak, "unit": "Gatomic/s", "frac": rate / peak, "traffic": traffic,
+            "traffic_source": src, "kernel": f"k_4pcf on {w['name']}", "launch_ms": launch_ms,
             "peak_kind": "global RED rate measured in this run (bench_peaks.cu)",
             "units_per_launch": {"hits": w["hits"], "red_per_hit": channels}}
 
@@ -468,7 +469,7 @@ def record_for(name, cats, args, peaks, hbm, hbm_kind, flush, steps, warmup, e2e
                                    frac=roofline_3pcf(name, dict(x), enum_ms[k], hbm, hbm_kind, peaks)["frac"])
                               for k, x in enumerate(work)]
     else:
-        roof = roofline_4pcf(w, enum_ms[dom], 1 if cats[dom]["weights"] is None else 2, peaks)
+        roof = roofline_4pcf(name, w, enum_ms[dom], 1 if cats[dom]["weights"] is None else 2, peaks)
     h2d = sum(c["points"].nbytes + (0 if c["weights"] is None else c["weights"].nbytes) for c in cats)
     nh = {"3pcf": 3, "4pcf": 6, "4pcf_parity": 6}
     d2h = sum(8 * c["nbins"] ** nh[c["kind"]] * (1 if c["weights"] is None else 2) * (2 if c["kind"] == "4pcf_parity" else 1)

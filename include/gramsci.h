@@ -40,7 +40,19 @@
  * DEVICE MEMORY.  The graph and all scratch come from the caller's allocator when gramsci_options.alloc /
  * dealloc are set (the Python binding can pass PyTorch's caching allocator), else from a private
  * stream-ordered memory pool of the device (never the device's default pool), which keeps freed blocks
- * for the next call; gramsci_release_memory() returns them to the driver.
+ * for the next call; gramsci_release_memory() returns them to the driver.  HOST MEMORY: only capped graphs use it
+ * (one page-locked block per window); freed blocks stay page-locked in a process-wide cache for the next capped
+ * build until gramsci_release_memory().
+ *
+ * ENVIRONMENT (test and ablation knobs, read at query time; none is needed for normal use):
+ *   GRAMSCI_FLUSH_BUDGET=n   drain the shared-memory histograms every n hits (parity tests force the drain paths)
+ *   GRAMSCI_CTA_KMAJOR=0     long-row gather kernel in its first loop order (one spoke per warp)
+ *   GRAMSCI_TILE_MB=n        spoke-tile size of the long-row gather kernel (default 64; forces tiling)
+ *   GRAMSCI_WMODE=1          weighted 3pCF sums as fixed-point limbs in shared memory instead of fp64 RED
+ *   GRAMSCI_4PCF_LUT=1       4pCF through the configuration look-up table and shared-memory histograms
+ *   GRAMSCI_OCC=n, GRAMSCI_CARVEOUT=p, GRAMSCI_HYBRID=1, GRAMSCI_GATHER_G=g   occupancy / carve-out / path experiments
+ *   GRAMSCI_TRIM_ON_FREE=1   trim the private device pool to 2 GiB when a graph larger than 4 GiB is freed
+ *   GRAMSCI_DEBUG=1          one line per query on stderr (kernel choice, sizes)
  */
 #ifndef GRAMSCI_H
 #define GRAMSCI_H
@@ -209,8 +221,10 @@ int gramsci_slab_range(const gramsci_graph *g, int32_t *hub_lo, int32_t *hub_hi)
 
 void gramsci_free_graph(gramsci_graph *g);
 
-/* Return the freed blocks of the library's private memory pool on the current device to the driver
- * (synchronises the device).  Graphs larger than 4 GiB trim the pool to 2 GiB when they are freed. */
+/* Return the freed blocks of the library's private memory pool on the current device to the driver and unpin the
+ * cached host blocks (synchronises the device).  Nothing is returned automatically: a freed graph's memory serves
+ * the next build (re-growing the pool for a 108 GB graph costs 2.6 s); call this before handing the device to
+ * another allocator.  GRAMSCI_TRIM_ON_FREE=1 restores trimming to 2 GiB whenever a graph larger than 4 GiB is freed. */
 int gramsci_release_memory(void);
 
 const char *gramsci_last_error(void); /* thread-local, never NULL */

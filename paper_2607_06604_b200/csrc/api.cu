@@ -73,6 +73,25 @@ static cudaMemPool_t gr_pool(int dev)
     return pool;
 }
 
+// device memory a new allocation of the library can draw on: what the driver reports free plus the freed blocks cached
+// in the private pool
+size_t gr_dev_available()
+{
+    size_t fr = 0, tot = 0;
+    if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fr;
+    cudaMemPool_t pool = gr_pool(dev);
+    if (pool) {
+        uint64_t res = 0, used = 0;
+        if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReservedMemCurrent, &res) == cudaSuccess &&
+            cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemCurrent, &used) == cudaSuccess && res > used)
+            fr += (size_t)(res - used);
+        cudaGetLastError();
+    }
+    return fr;
+}
+
 void *gr_dev_alloc(size_t bytes, const GrAllocCtx &ctx, int *kind)
 {
     void *p = nullptr;
@@ -86,7 +105,16 @@ void *gr_dev_alloc(size_t bytes, const GrAllocCtx &ctx, int *kind)
     GR_CUDA(cudaGetDevice(&dev));
     cudaMemPool_t pool = gr_pool(dev);
     if (pool) {
-        GR_CUDA(cudaMallocFromPoolAsync(&p, bytes, pool, ctx.stream));
+        cudaError_t e = cudaMallocFromPoolAsync(&p, bytes, pool, ctx.stream);
+        if (e == cudaErrorMemoryAllocation) {
+            // cached free blocks that do not fit this request (another size mix than the last graph's): give them back
+            // to the driver and try once more
+            cudaGetLastError();
+            cudaStreamSynchronize(ctx.stream);
+            cudaMemPoolTrimTo(pool, 0);
+            e = cudaMallocFromPoolAsync(&p, bytes, pool, ctx.stream);
+        }
+        GR_CUDA(e);
         *kind = 1;
     } else {
         GR_CUDA(cudaMalloc(&p, bytes));
@@ -395,10 +423,13 @@ extern "C" void gramsci_free_graph(gramsci_graph *g)
     if (!g) return;
     cudaStreamSynchronize(g->stream);
     for (auto &w : g->windows) { gr_pinned_free(w.h_block, w.h_block_bytes); w.h_block = nullptr; }
-    const bool big = (uint64_t)g->n_edges * 5 > ((uint64_t)4 << 30) && !g->actx.alloc;
+    // Freed blocks stay in the library's private pool for the next graph: growing the pool again costs more than the whole
+    // build (configs[4]: 108 GB of graph, 2.6 s of a 12.7 s step went into re-growing a trimmed pool).  They are invisible to
+    // other allocators (PyTorch's) until gramsci_release_memory(); GRAMSCI_TRIM_ON_FREE=1 trims to 2 GiB after graphs > 4 GiB.
+    const bool trim = (uint64_t)g->n_edges * 5 > ((uint64_t)4 << 30) && !g->actx.alloc && getenv("GRAMSCI_TRIM_ON_FREE");
     cudaStream_t st = g->stream;
     delete g;
-    if (big) {      // do not sit on tens of GB of freed blocks: other users of the device (PyTorch) cannot see them
+    if (trim) {
         int dev = 0;
         cudaStreamSynchronize(st);
         if (cudaGetDevice(&dev) == cudaSuccess) {

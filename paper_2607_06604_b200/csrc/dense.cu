@@ -246,8 +246,7 @@ bool gr_dense_prepare(gramsci_graph *g)
     if (!gr_dense_tables(g)) return false;
     if (g->ooc || d.bytes.p) return true;
     GrTimer t(g->stream);
-    size_t fr = 0, tot = 0;
-    GR_CUDA(cudaMemGetInfo(&fr, &tot));
+    const size_t fr = gr_dev_available();
     if ((size_t)d.total + ((size_t)2 << 30) > fr) {
         d.state = -1;
         d.why = "not enough free device memory for the dense rows";

@@ -51,6 +51,7 @@ GrAllocCtx &gr_alloc_ctx();
 inline cudaStream_t &gr_alloc_stream() { return gr_alloc_ctx().stream; }
 void *gr_dev_alloc(size_t bytes, const GrAllocCtx &ctx, int *kind);     // kind: 0 cudaMalloc, 1 pool, 2 hook
 void gr_dev_free(void *p, const GrAllocCtx &ctx, int kind);
+size_t gr_dev_available();                     // driver-free bytes + freed blocks cached in the private pool
 
 template <typename T>
 struct DevBuf {

@@ -129,6 +129,24 @@ __device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned r
 #ifndef G3_SPU
 #define G3_SPU 2
 #endif
+#ifndef G3_FLAT
+#define G3_FLAT 1
+#endif
+#ifndef G3_FLAT_U
+#define G3_FLAT_U 4
+#endif
+#ifndef G3_PADMUL
+#define G3_PADMUL 0
+#endif
+#ifndef G3_MINB
+#define G3_MINB 3
+#endif
+#ifndef G3_WMINB
+#define G3_WMINB 1
+#endif
+#ifndef G3_DUMMY_WARP
+#define G3_DUMMY_WARP 1
+#endif
 __device__ __forceinline__ void sred_inc_sel(unsigned a, unsigned bv, unsigned a_dummy)
 {
     asm volatile("{\n .reg .pred q;\n .reg .u32 a2;\n setp.ne.u32 q, %1, 255;\n selp.u32 a2, %0, %2, q;\n red.shared.add.u32 [a2], 1;\n}"
@@ -313,6 +331,62 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
             __syncwarp();
             const double wi = WMODE ? v.w[i] * (WMODE == 1 ? p.wscale : 1.0) : 0.0;
 
+            if (G3_FLAT && WMODE == 0) {      // (weighted launches run at the RED rate either way: measured 32.4 vs 31.6 ms)
+                // FLAT: the n (n - 1) / 2 wedges (a, t), a < t, as one index space, so that no lane idles on the triangular
+                // shape (rows of ~56 entries: 86 warp iterations over blocks of 32 entries, 49 over the flat space).  Spoke p
+                // (n - 1 - p wedges) and spoke n - 2 - p (p + 1 wedges) share a row of exactly n slots:
+                //      slot s -> p = s / n, x = s % n;   x < n - 1 - p ?  (a, t) = (p, x + p + 1)  :  (n - 2 - p, x)
+                // (s / n by a multiply-high with ceil(2^32 / n): exact while s n < 2^32; n <= 250 here)
+                const unsigned W = (unsigned)n * (unsigned)(n - 1) / 2u;
+                const unsigned M = 0xffffffffu / (unsigned)n + 1u;
+                constexpr int U = G3_FLAT_U;
+                for (unsigned s0 = 0; s0 < W; s0 += 32u * U) {
+                    uint2 sv[U], kv[U];
+                    unsigned off[U], bv[U];
+                    bool ok[U];
+                    double wa[U], wk[U];
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const unsigned sl = s0 + 32u * q + lane;
+                        ok[q] = sl < W;
+                        const unsigned pp = __umulhi(sl, M), x = sl - pp * (unsigned)n;
+                        const bool first = x < (unsigned)(n - 1) - pp;
+                        unsigned a = first ? pp : (unsigned)(n - 2) - pp;
+                        unsigned t = first ? x + pp + 1u : x;
+                        if (!ok[q]) { a = 0u; t = 0u; }
+                        sv[q] = lds_v2(a_sp + 8u * a);
+                        kv[q] = lds_v2(a_kx + 8u * t);
+                        if (WMODE) { wa[q] = lds_f64(a_aw + 8u * a); wk[q] = lds_f64(a_aw + 8u * t); }
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) off[q] = lds_u16(a_T + (kv[q].x >> 16) + (sv[q].y & 0x7c0u));
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        bool act = ok[q] && off[q] != T_NONE;
+                        if (OOC) act = act && sv[q].x != ROW_NONE;
+                        if (EQ) act = act && kv[q].y == (sv[q].y >> 11);
+                        bv[q] = 0xffu;
+                        if (act) bv[q] = ldg_u8(v.dense + ((size_t)sv[q].x << 5) + (off[q] + (kv[q].x & 0xffffu)));
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const unsigned hb = sv[q].y >> 11;               // byte offset of b_ij in the histogram (EQ: 4 b_ij)
+                        const unsigned ah = EQ ? a_hist + hb : a_hist + kv[q].y + hb + bv[q] * 4u;
+                        if (have_cnt) {
+                            if (G3_DUMMY_WARP && !EQ) sred_inc_sel(ah, bv[q], a_hist + 4u * (unsigned)p.nh);
+                            else sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
+                        }
+                        if (WMODE == 1) {
+                            unsigned l0, l1, l2;
+                            limbs_of((wi * wa[q]) * wk[q], l0, l1, l2);
+                            sred_limbs_hit<EQ>(ah + (have_cnt ? plane_b : 0u), plane_b, l0, l1, l2, bv[q], hb >> 2);
+                        } else if (WMODE == 2) {
+                            if (EQ ? (bv[q] == (hb >> 2)) : (bv[q] != 0xffu)) atomicAdd(&my_w[(ah - a_hist) >> 2], (wi * wa[q]) * wk[q]);
+                        }
+                    }
+                }
+                continue;
+            }
             // blocks of 32 tail entries (the lane's entry in registers); spokes a < min(n - 1, end of the block)
             for (int r0 = 0; r0 < n; r0 += 32) {
                 const int t = r0 + lane;
@@ -353,7 +427,10 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                     for (int q = 0; q < U; ++q) {
                         const unsigned hb = s[q].y >> 11;                // byte offset of b_ij in the histogram (EQ: 4 b_ij)
                         const unsigned ah = EQ ? a_hist + hb : a_hk + hb + bv[q] * 4u;
-                        if (have_cnt) sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
+                        if (have_cnt) {
+                            if (G3_DUMMY_WARP && !EQ) sred_inc_sel(ah, bv[q], a_hist + 4u * (unsigned)p.nh);
+                            else sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
+                        }
                         if (WMODE == 1 && p.hybrid && (q & 1)) {
                             if (EQ ? (bv[q] == (hb >> 2)) : (bv[q] != 0xffu))
                                 atomicAdd(&my_w[(ah - a_hist) >> 2], ((wi * wa[q]) * ak) * p.inv_wscale);
@@ -432,7 +509,7 @@ __device__ __forceinline__ void build_T_row32(const G3Tables &tb, int cj, int fc
 // the LSU wavefront rate (profiles/r2_gather_cta_cfg5e.md), so loads are what is worth removing.  Work items (chunk,
 // spoke block) are dealt to the warps through a shared-memory counter.
 template <int WMODE, bool EQ, bool OOC, bool KMAJOR>
-__global__ void __launch_bounds__(G3_THREADS)
+__global__ void __launch_bounds__(G3_THREADS, KMAJOR ? (WMODE == 0 ? G3_MINB : G3_WMINB) : 1)
 k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restrict__ unit_counter,
                   unsigned long long *__restrict__ g_cnt, double *__restrict__ g_w)
 {
@@ -620,8 +697,10 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     // pointing them at the 0xFF pad byte of the row instead costs more in sectors than the predicate does
                     // in issue slots: cfg5 1/8 replica 2.04 s against 1.91 s)
                     const uint8_t *pq[4];
+                    unsigned mulq[4];                                  // G3_PADMUL: 32, or 0 for an entry without a segment
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
+                        mulq[q] = 32u;
                         tq[q] = t0 + 32 * q + lane;
                         const unsigned kk = (tq[q] < n) ? lds_u32(a_kx + 4u * tq[q]) : (31u << 16);
                         pos[q] = kk & 0xffffu;
@@ -635,6 +714,13 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     auto gather = [&](int a, unsigned ea, auto TRIc, unsigned (&bv)[4]) {
                         constexpr bool TRI = decltype(TRIc)::value;
                         const unsigned rs = (ea & 0xffffu) * rl5;      // row of the spoke, in sectors from its cell's first row
+                        if (G3_PADMUL && !TRI && !EQ && !OOC) {
+                            // no predicate: an entry without a segment reads ONE fixed 0xFF byte per cell (the pad byte of the
+                            // cell's first row, multiplier 0), which stays in L1
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) bv[q] = ldg_u8(pq[q] + (size_t)rs * mulq[q]);
+                            return;
+                        }
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
                             bool act = pq[q] != nullptr;
@@ -682,6 +768,10 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                                 for (int q = 0; q < 4; ++q) {
                                     const unsigned o2 = lds_u32(a_Tj + okk[q]);
                                     pq[q] = (o2 == ROW_NONE) ? nullptr : cell_rows + (o2 + pos[q]);
+                                    if (G3_PADMUL && !TRI && !EQ && !OOC) {
+                                        mulq[q] = (o2 == ROW_NONE) ? 0u : 32u;
+                                        if (o2 == ROW_NONE) pq[q] = cell_rows + ((unsigned)f_rowlen[oj] - 1u);
+                                    }
                                 }
                             }
                             for (; a + SPU <= run_end; a += SPU) {

@@ -77,7 +77,7 @@ def test_roofline_arithmetic_reproduces_by_hand():
     t_l2 = (4 * 1.0e10 + 6.0e9) / 12000e9
     assert r["bound"] == "l2" and abs(r["frac"] - t_l2 * 1e3 / 20.0) < 1e-12
     assert abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-12
-    r4 = bench.roofline_4pcf(dict(name="y", hits=1.5e9), 10.0, 1, peaks)
+    r4 = bench.roofline_4pcf("x", dict(name="y", hits=1.5e9), 10.0, 1, peaks)
     assert r4["bound"] == "l2-atomics" and abs(r4["frac"] - (1.5e9 / 10e-3 / 1e9) / 185.0) < 1e-12
 
 
