@@ -135,9 +135,6 @@ __device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned r
 #ifndef G3_FLAT_U
 #define G3_FLAT_U 4
 #endif
-#ifndef G3_PADMUL
-#define G3_PADMUL 0
-#endif
 #ifndef G3_MINB
 #define G3_MINB 3
 #endif
@@ -694,13 +691,11 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     double wk[4];
                     // byte address of (first row of the spoke's cell) + (offset of the lane's entry in such a row); null for an
                     // entry whose cell is not forward of the spoke's (about half of the wedges: no load is issued for them --
-                    // pointing them at the 0xFF pad byte of the row instead costs more in sectors than the predicate does
-                    // in issue slots: cfg5 1/8 replica 2.04 s against 1.91 s)
+                    // pointing them at a 0xFF pad byte instead, of the spoke's row or one fixed byte per cell, was measured
+                    // slower: the predicate costs less in issue slots than the extra loads cost in the L1 data pipe)
                     const uint8_t *pq[4];
-                    unsigned mulq[4];                                  // G3_PADMUL: 32, or 0 for an entry without a segment
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
-                        mulq[q] = 32u;
                         tq[q] = t0 + 32 * q + lane;
                         const unsigned kk = (tq[q] < n) ? lds_u32(a_kx + 4u * tq[q]) : (31u << 16);
                         pos[q] = kk & 0xffffu;
@@ -714,13 +709,6 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     auto gather = [&](int a, unsigned ea, auto TRIc, unsigned (&bv)[4]) {
                         constexpr bool TRI = decltype(TRIc)::value;
                         const unsigned rs = (ea & 0xffffu) * rl5;      // row of the spoke, in sectors from its cell's first row
-                        if (G3_PADMUL && !TRI && !EQ && !OOC) {
-                            // no predicate: an entry without a segment reads ONE fixed 0xFF byte per cell (the pad byte of the
-                            // cell's first row, multiplier 0), which stays in L1
-#pragma unroll
-                            for (int q = 0; q < 4; ++q) bv[q] = ldg_u8(pq[q] + (size_t)rs * mulq[q]);
-                            return;
-                        }
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
                             bool act = pq[q] != nullptr;
@@ -768,10 +756,6 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                                 for (int q = 0; q < 4; ++q) {
                                     const unsigned o2 = lds_u32(a_Tj + okk[q]);
                                     pq[q] = (o2 == ROW_NONE) ? nullptr : cell_rows + (o2 + pos[q]);
-                                    if (G3_PADMUL && !TRI && !EQ && !OOC) {
-                                        mulq[q] = (o2 == ROW_NONE) ? 0u : 32u;
-                                        if (o2 == ROW_NONE) pq[q] = cell_rows + ((unsigned)f_rowlen[oj] - 1u);
-                                    }
                                 }
                             }
                             for (; a + SPU <= run_end; a += SPU) {
