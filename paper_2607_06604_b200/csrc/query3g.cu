@@ -1020,10 +1020,11 @@ void gr_3pcf_gather(gramsci_graph *g, uint64_t *d_counts, double *d_wsum, int eq
         if (un.n == 0) continue;
         if (r.smem > g->smem_optin)
             GR_FAIL(GRAMSCI_ERANGE, "3pcf (gather): histogram or longest row (%d entries) does not fit in shared memory", g->max_row);
-        // long rows: lanes keep their tail entries, the loop runs over the spokes (KMAJOR); GRAMSCI_CTA_KMAJOR=0 selects the
-        // spoke-per-warp loop (kept for the ablation); the limb path (WMODE 1) needs its mid-hub drains and stays there
-        int kmajor = (wmode != 1 && g->max_row <= 65000) ? 1 : 0;
-        if (const char *e = getenv("GRAMSCI_CTA_KMAJOR")) kmajor = kmajor && atoi(e) != 0;
+        // long rows: lanes keep their tail entries, the loop runs over the spokes (KMAJOR) for counts; weighted launches
+        // run at the RED rate in either order and the first one is slightly ahead (cfg2-D 31.0 vs 31.8 ms);
+        // GRAMSCI_CTA_KMAJOR=0 / 1 forces an order (ablation, tests); the limb path (WMODE 1) needs its mid-hub drains
+        int kmajor = (wmode == 0 && g->max_row <= 65000) ? 1 : 0;
+        if (const char *e = getenv("GRAMSCI_CTA_KMAJOR")) kmajor = (atoi(e) != 0 && wmode != 1 && g->max_row <= 65000) ? 1 : 0;
         r.fn = gather_fn(wmode, r.eq, (k && kmajor) ? 2 : k, g->ooc);
         if (const char *e = getenv("GRAMSCI_CARVEOUT"))      // experiment: shared-memory carve-out in percent (L1 gets the rest)
             cudaFuncSetAttribute((const void *)r.fn, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(e));

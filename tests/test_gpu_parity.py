@@ -457,6 +457,13 @@ def test_gather_cta_loop_orders(kmajor, monkeypatch):
         assert gg.info()["max_row"] > 2000
         assert np.array_equal(gg.pcf3()[0], oc)
         assert np.array_equal(gg.pcf3_equilateral()[0], oc.reshape(18, 18, 18)[np.arange(18), np.arange(18), np.arange(18)])
+    # slab + halo graphs on long rows (hub range inside the CTA kernel): two slabs add up
+    tot = np.zeros_like(oc)
+    for rank in range(2):
+        gs = gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], algo=gr.ALGO_GATHER,
+                                    slab_count=2, slab_index=rank)
+        tot += gs.pcf3()[0]
+    assert np.array_equal(tot, oc)
     c5 = cat.config5(seed=5102, n=3_000, L=310.0)
     w = np.random.default_rng(9).uniform(0.5, 1.5, 3000)
     og = oracle.Graph(c5["points"], w, c5["box"], c5["r_min"], c5["r_max"], c5["nbins"])
