@@ -496,6 +496,43 @@ def record_for(name, cats, args, peaks, hbm, hbm_kind, flush, steps, warmup, e2e
     return rec
 
 
+def run_shard_sweep(args):
+    """--shard-sweep 2,4,8: the N slab + halo graphs of ONE workload built and queried ONE AFTER THE OTHER on this GPU.
+    This measures the work partition (stored edges, enumeration time and its imbalance per shard count, shards summing to
+    the full histogram) -- NOT a scaling curve: no two ranks ever run at the same time."""
+    import torch
+    import paper_2607_06604_b200 as gr
+    torch.cuda.set_device(0)
+    gr.load_library()
+    c = workload(args.workload)[0]
+    pts = torch.from_numpy(c["points"]).cuda()
+    w = None if c["weights"] is None else torch.from_numpy(c["weights"]).cuda()
+
+    def one(**part):
+        g = gr.gramsci_build_graph(pts, w, c["box"], c["r_min"], c["r_max"], c["nbins"], algo=args.algo, **part)
+        cnt, _ = g.pcf3()
+        rec = dict(build_ms=g.timing(0), enum_ms=g.timing(2), query_ms=g.timing(1), stored_edges=g.info()["n_edges"],
+                   hubs=g.slab_range())
+        g.free()
+        return cnt, rec
+    full, base = one()
+    out = {"workload": args.workload, "note": "shards run sequentially on one GPU: work partition, not a scaling measurement",
+           "partition": args.partition, "full": base, "sweeps": []}
+    for n in [int(x) for x in args.shard_sweep.split(",") if x]:
+        tot, recs = np.zeros_like(full), []
+        for r in range(n):
+            part = dict(slab_count=n, slab_index=r) if args.partition == "slab" else dict(shard_count=n, shard_index=r)
+            cnt, rec = one(**part)
+            tot += cnt
+            recs.append(rec)
+        en = [x["enum_ms"] for x in recs]
+        out["sweeps"].append({"n_shards": n, "sum_equals_full": bool(np.array_equal(tot, full)), "enum_ms": en,
+                              "enum_imbalance": imbalance(en), "ideal_speedup": n, "speedup_bound_from_max_shard": base["enum_ms"] / max(en),
+                              "stored_edges_fraction": [x["stored_edges"] / base["stored_edges"] for x in recs],
+                              "build_ms": [x["build_ms"] for x in recs]})
+    print(json.dumps(out))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -592,7 +629,13 @@ def main():
     ap.add_argument("--skip-e2e", action="store_true", help="no host-buffer leg (e2e = null)")
     ap.add_argument("--cap-gib", type=float, default=0.0,
                     help="device_mem_cap_bytes in GiB (0 = whole CSR resident); forces the out-of-core tiler")
+    ap.add_argument("--shard-sweep", default="",
+                    help="e.g. 2,4,8: build and query the N shards of the workload one after the other on ONE GPU (work "
+                         "partition and imbalance of --partition; not a scaling measurement)")
     args = ap.parse_args()
+    if args.shard_sweep:
+        run_shard_sweep(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:
