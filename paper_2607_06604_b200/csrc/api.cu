@@ -238,8 +238,24 @@ void *gr_pinned_alloc(size_t *bytes)
 void gr_pinned_free(void *p, size_t bytes)
 {
     if (!p) return;
-    std::lock_guard<std::mutex> lk(g_pin_mu);
-    g_pin_cache.push_back({p, (bytes + 4095) & ~size_t(4095)});
+    std::vector<PinnedBlock> evict;
+    {
+        std::lock_guard<std::mutex> lk(g_pin_mu);
+        g_pin_cache.push_back({p, (bytes + 4095) & ~size_t(4095)});
+        // bound what stays page-locked: 64 GiB (one capped configs[4] graph is 42 GB); the oldest blocks go first
+        size_t total = 0;
+        for (auto &b : g_pin_cache) total += b.bytes;
+        while (total > (size_t(64) << 30) && g_pin_cache.size() > 1) {
+            evict.push_back(g_pin_cache.front());
+            total -= g_pin_cache.front().bytes;
+            g_pin_cache.erase(g_pin_cache.begin());
+        }
+    }
+    for (auto &b : evict) {
+        cudaHostUnregister(b.p);
+        munmap(b.p, b.bytes);
+    }
+    if (!evict.empty()) cudaGetLastError();
 }
 
 void gr_pinned_release_cache()

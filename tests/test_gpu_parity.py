@@ -805,7 +805,7 @@ def test_slab_and_halo_partition_adds_up(periodic, algo):
     n = cfg["points"].shape[0]
     for world in (2, 5):
         c2 = np.zeros_like(oc2); w2 = np.zeros_like(ow2); c3 = np.zeros_like(oc3); w3 = np.zeros_like(ow3)
-        c4 = np.zeros_like(oc4); w4 = np.zeros_like(ow4); cc3 = np.zeros_like(oc3)
+        c4 = np.zeros_like(oc4); w4 = np.zeros_like(ow4); cc3 = np.zeros_like(oc3); cc4 = np.zeros_like(oc4)
         cover, stored = [], []
         for rank in range(world):
             g = gr.gramsci_build_graph(cfg["points"], cfg["weights"], cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"],
@@ -821,6 +821,8 @@ def test_slab_and_halo_partition_adds_up(periodic, algo):
                                         slab_count=world, slab_index=rank, algo=algo, device_mem_cap_bytes=max(csr, 4096) * 2,
                                         n_windows=3)
             cc3 += gc.pcf3()[0]
+            if world == 2:                                           # 4pCF tiles (h, c1 <= c2) on a capped slab graph
+                cc4 += gc.pcf4()[0]
             gc.free()
         assert cover[0][0] == 0 and cover[-1][1] == n and all(cover[k][1] == cover[k + 1][0] for k in range(world - 1))
         assert all(hi > lo for lo, hi in cover)                      # every slab got hubs (work-balanced cut)
@@ -828,6 +830,7 @@ def test_slab_and_halo_partition_adds_up(periodic, algo):
         if world == 5:
             assert max(stored) < 0.6 * og.n_edges                    # slab + halo, not the whole graph
         assert np.array_equal(c2, oc2) and np.array_equal(c3, oc3) and np.array_equal(c4, oc4) and np.array_equal(cc3, oc3)
+        assert world != 2 or np.array_equal(cc4, oc4)
         assert_weighted_close(w2, ow2); assert_weighted_close(w3, ow3); assert_weighted_close(w4, ow4)
     with pytest.raises(gr.GramsciError):                             # needs cell-order labels
         gr.gramsci_build_graph(cfg["points"], None, cfg["box"], cfg["r_min"], cfg["r_max"], cfg["nbins"], slab_count=2, relabel=2)
