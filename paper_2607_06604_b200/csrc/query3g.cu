@@ -289,6 +289,8 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
         cb = wb = 0;
     };
 
+    const uint8_t *dbase = v.dense;              // kept in registers (otherwise re-read from the constant bank at every gather)
+    asm volatile("" : "+l"(dbase));
     int cur_cell = -1;
     for (;;) {
         int u = 0;
@@ -344,13 +346,13 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                     double wa[U], wk[U];
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
-                        const unsigned sl = s0 + 32u * q + lane;
+                        unsigned sl = s0 + 32u * q + lane;
                         ok[q] = sl < W;
+                        sl = min(sl, W - 1u);                            // a slot beyond the end re-reads the last wedge (masked below)
                         const unsigned pp = __umulhi(sl, M), x = sl - pp * (unsigned)n;
                         const bool first = x < (unsigned)(n - 1) - pp;
-                        unsigned a = first ? pp : (unsigned)(n - 2) - pp;
-                        unsigned t = first ? x + pp + 1u : x;
-                        if (!ok[q]) { a = 0u; t = 0u; }
+                        const unsigned a = first ? pp : (unsigned)(n - 2) - pp;
+                        const unsigned t = first ? x + pp + 1u : x;
                         sv[q] = lds_v2(a_sp + 8u * a);
                         kv[q] = lds_v2(a_kx + 8u * t);
                         if (WMODE) { wa[q] = lds_f64(a_aw + 8u * a); wk[q] = lds_f64(a_aw + 8u * t); }
@@ -363,7 +365,7 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                         if (OOC) act = act && sv[q].x != ROW_NONE;
                         if (EQ) act = act && kv[q].y == (sv[q].y >> 11);
                         bv[q] = 0xffu;
-                        if (act) bv[q] = ldg_u8(v.dense + ((size_t)sv[q].x << 5) + (off[q] + (kv[q].x & 0xffffu)));
+                        if (act) bv[q] = ldg_u8(dbase + ((size_t)sv[q].x << 5) + (off[q] + (kv[q].x & 0xffffu)));
                     }
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
