@@ -865,39 +865,49 @@ void gr_build(gramsci_graph *g, const double *d_points, const double *d_weights,
         GR_CUDA(cudaMemcpyAsync(hptr.data(), g->ptr.p, sizeof(int64_t) * (n + 1), cudaMemcpyDeviceToHost, st));
         GR_CUDA(cudaStreamSynchronize(st));
     }
-    if (W <= 1) {
-        GrWindow w0;
-        w0.row_lo = 0; w0.row_hi = (int32_t)n; w0.e_lo = 0; w0.e_hi = E;
-        g->windows.push_back(w0);
-    } else {
-        // boundaries at the first row starting at or after k*E/W (k = 1..W-1); empty windows are dropped
-        int32_t r = 0;
-        for (int k = 1; k <= W && r < n; ++k) {
-            int32_t r2 = (int32_t)n;
-            if (k < W) {
-                const int64_t want = (int64_t)(((__int128)E * k) / W);
-                r2 = (int32_t)(std::lower_bound(hptr.begin(), hptr.begin() + n, want) - hptr.begin());
-                r2 = std::max(r2, r + 1);
-                r2 = (int32_t)std::min<int64_t>(r2, n);
-                if (hptr[r2] == hptr[r] && r2 < n) continue;      // no edges yet: extend this window
+    // The cut is by edges, the buffers also hold dense rows, and a window cannot split a row: the largest window can exceed
+    // cap / 4.  W grows until FOUR buffers fit (hub + search + the next tile's two: with three the tiler re-stages a window
+    // for nearly every tile -- configs[4] under 24 GiB: 114 GB staged per query with 3 buffers, 1.3 x the CSR with 4).
+    for (int attempt = 0;; ++attempt) {
+        g->windows.clear();
+        if (W <= 1) {
+            GrWindow w0;
+            w0.row_lo = 0; w0.row_hi = (int32_t)n; w0.e_lo = 0; w0.e_hi = E;
+            g->windows.push_back(w0);
+        } else {
+            // boundaries at the first row starting at or after k*E/W (k = 1..W-1); empty windows are dropped
+            int32_t r = 0;
+            for (int k = 1; k <= W && r < n; ++k) {
+                int32_t r2 = (int32_t)n;
+                if (k < W) {
+                    const int64_t want = (int64_t)(((__int128)E * k) / W);
+                    r2 = (int32_t)(std::lower_bound(hptr.begin(), hptr.begin() + n, want) - hptr.begin());
+                    r2 = std::max(r2, r + 1);
+                    r2 = (int32_t)std::min<int64_t>(r2, n);
+                    if (hptr[r2] == hptr[r] && r2 < n) continue;      // no edges yet: extend this window
+                }
+                GrWindow w;
+                w.row_lo = r;
+                w.row_hi = r2;
+                w.e_lo = hptr[r] & ~int64_t(15);
+                w.e_hi = hptr[r2];
+                g->windows.push_back(w);
+                r = r2;
             }
-            GrWindow w;
-            w.row_lo = r;
-            w.row_hi = r2;
-            w.e_lo = hptr[r] & ~int64_t(15);
-            w.e_hi = hptr[r2];
-            g->windows.push_back(w);
-            r = r2;
         }
-    }
-
-    if (g->ooc && g->spatial && gr_dense_tables(g)) {      // dense byte range of every window
-        std::vector<int32_t> rows;
-        for (auto &w : g->windows) rows.push_back(w.row_lo);
-        rows.push_back((int32_t)n);
-        std::vector<int64_t> addr(rows.size());
-        gr_dense_rowaddrs(g, rows.data(), (int)rows.size(), addr.data());
-        for (size_t k = 0; k < g->windows.size(); ++k) { g->windows[k].d_lo = addr[k]; g->windows[k].d_hi = addr[k + 1]; }
+        if (g->ooc && g->spatial && gr_dense_tables(g)) {      // dense byte range of every window
+            std::vector<int32_t> rows;
+            for (auto &w : g->windows) rows.push_back(w.row_lo);
+            rows.push_back((int32_t)n);
+            std::vector<int64_t> addr(rows.size());
+            gr_dense_rowaddrs(g, rows.data(), (int)rows.size(), addr.data());
+            for (size_t k = 0; k < g->windows.size(); ++k) { g->windows[k].d_lo = addr[k]; g->windows[k].d_hi = addr[k + 1]; }
+        }
+        if (!g->ooc || n_windows_forced > 0 || attempt >= 12 || W >= 1000) break;
+        int64_t maxbuf = 0;
+        for (auto &w : g->windows) maxbuf = std::max<int64_t>(maxbuf, (w.e_hi - w.e_lo) * (int64_t)bpe + (w.d_hi - w.d_lo));
+        if ((uint64_t)maxbuf * 4 <= g->cap_bytes) break;
+        W = W + std::max(1, W / 8);
     }
 
     DevBuf<int32_t> stats;
