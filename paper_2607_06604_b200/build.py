@@ -2,6 +2,9 @@
 
 Usage: python -m paper_2607_06604_b200.build [--force]
 The .so is git-ignored but travels to the GPU box with the gpurun snapshot.
+GRAMSCI_NVCC_DEFS adds compiler flags, e.g. the bounds-checked debug build (every dense-row gather and shared-memory
+histogram address of the gather kernels checked, a violation traps):
+    GRAMSCI_NVCC_DEFS=-DG3_BOUNDS=1 python -m paper_2607_06604_b200.build --force && python -m pytest tests -m gpu
 """
 from __future__ import annotations
 
@@ -44,7 +47,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     for s in SOURCES:
         o = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [_nvcc(), *NVCC_FLAGS, "-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("GRAMSCI_NVCC_DEFS", "").split(), "-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(o)
     log = []

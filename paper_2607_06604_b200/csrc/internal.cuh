@@ -225,6 +225,7 @@ struct GrView {
     int32_t shard_count, shard_index;   // shard_count > 1: only hubs with label % shard_count == shard_index
     // dense cell-block rows of the resident search rows (gather kernel): row of label j at dense + rowaddr(j) - d0
     const uint8_t *dense; int64_t d0;
+    int64_t dense_span;     // bytes of dense rows behind `dense` (bounds checks of the debug build, -DG3_BOUNDS=1)
 };
 
 void gr_2pcf(gramsci_graph *g, uint64_t *d_counts, double *d_wsum);

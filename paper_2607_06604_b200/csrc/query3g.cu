@@ -101,6 +101,13 @@ __device__ __forceinline__ double lds_f64(unsigned a)
 }
 // one byte of a dense row through the read-only path, zero-extended into a 32-bit register (opaque to the compiler, which
 // otherwise re-masks the byte before every use)
+// -DG3_BOUNDS=1 (debug build; compute-sanitizer is not available on the GPU pool): every gather address is checked
+// against the dense rows behind the view and every histogram address against the CTA's planes; a violation traps
+#ifndef G3_BOUNDS
+#define G3_BOUNDS 0
+#endif
+#define G3_CHECK_DENSE(v, ptr) do { if (G3_BOUNDS && ((ptr) < (v).dense || (ptr) >= (v).dense + (v).dense_span)) __trap(); } while (0)
+#define G3_CHECK_HIST(a, lo, bytes) do { if (G3_BOUNDS && ((a) < (lo) || (a) >= (lo) + (bytes) || ((a) & 3u))) __trap(); } while (0)
 __device__ __forceinline__ unsigned ldg_u8(const uint8_t *p)
 {
     unsigned v;
@@ -365,13 +372,18 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                         if (OOC) act = act && sv[q].x != ROW_NONE;
                         if (EQ) act = act && kv[q].y == (sv[q].y >> 11);
                         bv[q] = 0xffu;
-                        if (act) bv[q] = ldg_u8(dbase + ((size_t)sv[q].x << 5) + (off[q] + (kv[q].x & 0xffffu)));
+                        if (act) {
+                            const uint8_t *ptr = dbase + ((size_t)sv[q].x << 5) + (off[q] + (kv[q].x & 0xffffu));
+                            G3_CHECK_DENSE(v, ptr);
+                            bv[q] = ldg_u8(ptr);
+                        }
                     }
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
                         const unsigned hb = sv[q].y >> 11;               // byte offset of b_ij in the histogram (EQ: 4 b_ij)
                         const unsigned ah = EQ ? a_hist + hb : a_hist + kv[q].y + hb + bv[q] * 4u;
                         if (have_cnt) {
+                            if (bv[q] != 0xffu) G3_CHECK_HIST(ah, a_hist, 4u * (unsigned)p.nh);
                             if (G3_DUMMY_WARP && !EQ) sred_inc_sel(ah, bv[q], a_hist + 4u * (unsigned)p.nh);
                             else sred_inc_hit<EQ>(ah, bv[q], hb >> 2);
                         }
@@ -420,7 +432,10 @@ k_3pcf_gather_warp(GrView v, G3Params p, G3Tables tb, unsigned long long *__rest
                         if (TRI) act = act && t > a0 + q;
                         if (EQ) act = act && kxv.y == (s[q].y >> 11);
                         bv[q] = 0xffu;
-                        if (act) bv[q] = __ldg(v.dense + ((size_t)s[q].x << 5) + (off[q] + pk));
+                        if (act) {
+                            G3_CHECK_DENSE(v, v.dense + ((size_t)s[q].x << 5) + (off[q] + pk));
+                            bv[q] = __ldg(v.dense + ((size_t)s[q].x << 5) + (off[q] + pk));
+                        }
                     }
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
@@ -717,7 +732,10 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                             if (TRI) act = act && tq[q] > a;
                             if (EQ) act = act && hk[q] == (ea >> 21);
                             bv[q] = 0xffu;
-                            if (act) bv[q] = ldg_u8(pq[q] + (size_t)rs * 32u);
+                            if (act) {
+                                G3_CHECK_DENSE(v, pq[q] + (size_t)rs * 32u);
+                                bv[q] = ldg_u8(pq[q] + (size_t)rs * 32u);
+                            }
                         }
                     };
                     // ... and its four histogram updates
@@ -729,6 +747,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                         for (int q = 0; q < 4; ++q) {
                             const unsigned ah = EQ ? a_hj : a_hj + hk[q] + bv[q] * 4u;
                             if (have_cnt) {
+                                if (bv[q] != 0xffu) G3_CHECK_HIST(ah, a_hist, 4u * (unsigned)p.nh);
                                 if (G3_DUMMY_BIN && !EQ) sred_inc_sel(ah, bv[q], a_hist + 4u * (unsigned)p.nh);
                                 else sred_inc_hit<EQ>(ah, bv[q], ba);
                             }
@@ -822,7 +841,10 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                         bool act = off[q] != ROW_NONE;
                         if (EQ) act = act && (kk[q] >> 21) == ba;
                         bv[q] = 0xffu;
-                        if (act) bv[q] = __ldg(row + (off[q] + (kk[q] & 0xffffu)));
+                        if (act) {
+                            G3_CHECK_DENSE(v, row + (off[q] + (kk[q] & 0xffffu)));
+                            bv[q] = __ldg(row + (off[q] + (kk[q] & 0xffffu)));
+                        }
                     }
 #pragma unroll
                     for (int q = 0; q < U; ++q) {

@@ -49,6 +49,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     v.shard_index = g->shard_index;
     v.dense = g->dn.bytes.p;
     v.d0 = 0;
+    v.dense_span = g->dn.total;
     if (!g->ooc) {
         v.idx_h = v.idx_c = g->idx.p;
         v.bin_h = v.bin_c = g->bin.p;
@@ -180,6 +181,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
         v.c2_lo = wc2.row_lo; v.c2_hi = wc2.row_hi;
         v.dense = need_dense ? slots[b].dense.p : nullptr;
         v.d0 = wc.d_lo;
+        v.dense_span = wc.d_hi - wc.d_lo;
         if (g->spatial) { v.s_lo = v.h_lo; v.s_hi = v.h_hi; }
         else { v.s_lo = 0; v.s_hi = (int32_t)g->n; }
         if (v.h_hi > v.h_lo) fn(g, v, user, st);
