@@ -81,6 +81,21 @@ def test_roofline_arithmetic_reproduces_by_hand():
     assert r4["bound"] == "l2-atomics" and abs(r4["frac"] - (1.5e9 / 10e-3 / 1e9) / 185.0) < 1e-12
 
 
+def test_traffic_comes_from_the_committed_capture():
+    """roofline.traffic = DRAM bytes of the launch from profiles/dram_traffic.json, whose sources are committed csv files."""
+    import json
+    import bench
+    table = json.load(open(os.path.join(ROOT, "profiles", "dram_traffic.json")))
+    for key in ("cfg5:cfg5", "cfg2:cfg2D", "cfg2:cfg2R", "cfg3:cfg3"):
+        b, src = bench.dram_traffic(key)
+        assert b == table[key]["bytes"] > 0 and src.startswith("profiles/dram_traffic.json")
+        assert os.path.exists(os.path.join(ROOT, "profiles", table[key]["source"].split(" ")[0]))
+    assert bench.dram_traffic("nothing:here") == (None, None)
+    w = dict(name="cfg5", weighted=False, edges=8.4e9, spoke=1.8e13, tail=1.4e13, hits=7.1e12)
+    peaks = dict(l2_read_gbs=13500.0, smem_atom_gops=2000.0, red_f64_gops=190.0, red_u64_gops=185.0)
+    assert bench.roofline_3pcf("cfg5", w, 9560.0, 6465.0, "test", peaks)["traffic"] == table["cfg5:cfg5"]["bytes"]
+
+
 def test_reference_arm_line_schema():
     """bench.py --impl reference (the oracle on the host cores) prints one JSON line with the contract's keys."""
     import json
