@@ -142,6 +142,9 @@ __device__ __forceinline__ void sred_inc_hit(unsigned a, unsigned bv, unsigned r
 #ifndef G3_FLAT_U
 #define G3_FLAT_U 4
 #endif
+#ifndef G3_SBLK
+#define G3_SBLK 128          /* spokes per work item of the k-major loop */
+#endif
 #ifndef G3_MINB
 #define G3_MINB 3
 #endif
@@ -686,7 +689,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     for (int c = 0; c < n_chunks; ++c) {
                         s_cum[c] = cum;
                         const int a_end = min(a_hi, min(n, t_base + 128 * c + 128) - 1);
-                        cum += (a_end - a_lo + 31) >> 5;
+                        cum += (a_end - a_lo + G3_SBLK - 1) / G3_SBLK;
                     }
                     s_cum[n_chunks] = cum;
                     s_item = 0;
@@ -702,7 +705,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     while (s_cum[c + 1] <= item) ++c;                  // items come in ascending order
                     const int t0 = t_base + 128 * c;
                     const int a_end = min(a_hi, min(n, t0 + 128) - 1);
-                    const int sa = a_lo + 32 * (item - s_cum[c]), sb = min(a_end, sa + 32);
+                    const int sa = a_lo + G3_SBLK * (item - s_cum[c]), sb = min(a_end, sa + G3_SBLK);
                     unsigned pos[4], okk[4], hk[4];
                     int tq[4];
                     double wk[4];
