@@ -219,6 +219,22 @@ int gramsci_work_counters(const gramsci_graph *g, uint64_t *spoke_elems, uint64_
  * [0, N) unless the graph was built with slab_count > 1. */
 int gramsci_slab_range(const gramsci_graph *g, int32_t *hub_lo, int32_t *hub_hi);
 
+/*
+ * The 2pCF sweep WITHOUT ANY ALLOCATION (csrc/noalloc.cu), for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it.  Same result as gramsci_2pcf.  The accumulators live in a static
+ * device array of GRAMSCI_NOALLOC_MAX_BINS bins (2 KB, held by every GPU that loads the library until exit).
+ *   - counts [nb] uint64, wsum [nb] fp64: DEVICE buffers on the current device (either may be NULL); host buffers are
+ *     rejected (staging them would allocate).  The graph must be resident (no device_mem_cap_bytes) and on the current
+ *     device.  EINVAL with a message for nbins > GRAMSCI_NOALLOC_MAX_BINS, capped graphs, host outputs.
+ *   - The call ENQUEUES memset + kernel + copies on the graph's stream and does NOT synchronise (no allocation, no event,
+ *     no synchronisation: capturable): the outputs are complete once that stream has been synchronised by the caller.
+ *     The first call on a device looks up the array's address (cudaGetSymbolAddress): make it once outside a capture.
+ *   - All calls on a device share the array (cleared at the start of each call): calls that overlap on the GPU -- different
+ *     streams with no ordering between them -- race on it.  Calls on one stream, one after the other, are safe.
+ */
+#define GRAMSCI_NOALLOC_MAX_BINS 128
+int gramsci_2pcf_noalloc(const gramsci_graph *g, uint64_t *counts, double *wsum);
+
 void gramsci_free_graph(gramsci_graph *g);
 
 /* Return the freed blocks of the library's private memory pool on the current device to the driver and unpin the

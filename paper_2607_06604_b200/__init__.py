@@ -26,7 +26,10 @@ ABI_SYMBOLS = [
     "gramsci_4pcf", "gramsci_4pcf_parity", "gramsci_num_configs", "gramsci_compact", "gramsci_zeta_disc",
     "gramsci_last_timing", "gramsci_work_counters", "gramsci_free_graph", "gramsci_last_error",
     "gramsci_export_labels", "gramsci_release_memory", "gramsci_3pcf_equilateral", "gramsci_slab_range",
+    "gramsci_2pcf_noalloc",
 ]
+
+NOALLOC_MAX_BINS = 128          # GRAMSCI_NOALLOC_MAX_BINS of include/gramsci.h (gramsci_2pcf_noalloc)
 
 ALGO_DEFAULT, ALGO_MERGEPATH, ALGO_BSEARCH, ALGO_BITMAP = 0, 1, 2, 3
 ALGO_TABLE_G1, ALGO_TABLE_G2, ALGO_TABLE_G4, ALGO_TABLE_G8 = 4, 5, 6, 7
@@ -116,6 +119,8 @@ def load_library():
     L.gramsci_export_labels.argtypes = [vp, vp]
     L.gramsci_release_memory.restype = ctypes.c_int
     L.gramsci_release_memory.argtypes = []
+    L.gramsci_2pcf_noalloc.restype = ctypes.c_int
+    L.gramsci_2pcf_noalloc.argtypes = [vp] * 3
     L.gramsci_slab_range.restype = ctypes.c_int
     L.gramsci_slab_range.argtypes = [vp, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_int32)]
     _lib = L
@@ -227,6 +232,17 @@ class Graph:
         w = self._out(nb, "float64", host) if weighted else None
         _check(load_library().gramsci_2pcf(self._h, _ptr(c), _ptr(w)))
         return self._np(c), self._np(w)
+
+    def pcf2_noalloc(self, counts=None, wsum=None):
+        """``gramsci_2pcf_noalloc``: the 2pCF into the caller's CUDA tensors (int64 / float64 [nbins], either may be None)
+        with no allocation inside the library.  The call only ENQUEUES work on the graph's stream; this wrapper then
+        synchronises that stream (torch's current stream at build time) so that the tensors are complete on return."""
+        import torch
+        for t, dt in ((counts, torch.int64), (wsum, torch.float64)):
+            assert t is None or (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() >= self.nbins)
+        _check(load_library().gramsci_2pcf_noalloc(self._h, _ptr(counts), _ptr(wsum)))
+        torch.cuda.synchronize()
+        return counts, wsum
 
     def pcf3(self, counts: bool = True, weighted: bool = False, host: bool = False):
         nh = self.nbins ** 3

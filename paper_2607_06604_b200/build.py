@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgramsci.so")
-SOURCES = ["api.cu", "build_graph.cu", "dense.cu", "query3.cu", "query3g.cu", "query4.cu", "tiler.cu"]
+SOURCES = ["api.cu", "build_graph.cu", "dense.cu", "noalloc.cu", "query3.cu", "query3g.cu", "query4.cu", "tiler.cu"]
 HEADERS = [os.path.join(CSRC, "internal.cuh"), os.path.join(HERE, "..", "include", "gramsci.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
