@@ -709,11 +709,14 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     unsigned pos[4], okk[4], hk[4];
                     int tq[4];
                     double wk[4];
-                    // byte address of (first row of the spoke's cell) + (offset of the lane's entry in such a row); null for an
+                    // offset of the lane's entry inside a dense row of the spoke's cell (32 bits; the rows of the cell start at
+                    // cell_rows, which is warp-uniform and kept as ONE 64-bit pointer: with a 64-bit pointer per entry the
+                    // compiler spent two register moves per gather on pairing them up for IMAD.WIDE); ROW_NONE for an
                     // entry whose cell is not forward of the spoke's (about half of the wedges: no load is issued for them --
                     // pointing them at a 0xFF pad byte instead, of the spoke's row or one fixed byte per cell, was measured
                     // slower: the predicate costs less in issue slots than the extra loads cost in the L1 data pipe)
-                    const uint8_t *pq[4];
+                    unsigned pq[4];
+                    const uint8_t *cell_rows = v.dense;
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         tq[q] = t0 + 32 * q + lane;
@@ -721,7 +724,7 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                         pos[q] = kk & 0xffffu;
                         okk[q] = (kk >> 14) & 0x7cu;
                         hk[q] = EQ ? (kk >> 21) : (kk >> 21) * nb4;
-                        pq[q] = nullptr;
+                        pq[q] = ROW_NONE;
                         if (WMODE) wk[q] = (tq[q] < n) ? lds_f64(a_aw + 8u * tq[q]) : 0.0;
                     }
                     unsigned rl5 = 0;                                  // row length of the spoke's cell in 32-byte sectors
@@ -729,15 +732,17 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                     auto gather = [&](int a, unsigned ea, auto TRIc, unsigned (&bv)[4]) {
                         constexpr bool TRI = decltype(TRIc)::value;
                         const unsigned rs = (ea & 0xffffu) * rl5;      // row of the spoke, in sectors from its cell's first row
+                        const uint8_t *rowp = cell_rows + (size_t)rs * 32u;
+                        asm volatile("" : "+l"(rowp));                 // one 64-bit row pointer per spoke (not re-associated into the gathers)
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
-                            bool act = pq[q] != nullptr;
+                            bool act = pq[q] != ROW_NONE;
                             if (TRI) act = act && tq[q] > a;
                             if (EQ) act = act && hk[q] == (ea >> 21);
                             bv[q] = 0xffu;
                             if (act) {
-                                G3_CHECK_DENSE(v, pq[q] + (size_t)rs * 32u);
-                                bv[q] = ldg_u8(pq[q] + (size_t)rs * 32u);
+                                G3_CHECK_DENSE(v, rowp + pq[q]);
+                                bv[q] = ldg_u8(rowp + pq[q]);
                             }
                         }
                     };
@@ -774,12 +779,12 @@ k_3pcf_gather_cta(GrView v, G3Params p, G3Tables tb, unsigned long long *__restr
                             const int run_end = min(a_to, s_cf[oj + 1]);
                             {
                                 const unsigned a_Tj = a_T + (unsigned)oj * 128u;
-                                const uint8_t *cell_rows = v.dense + (f_dbase[oj] - v.d0);
+                                cell_rows = v.dense + (f_dbase[oj] - v.d0);
                                 rl5 = (unsigned)f_rowlen[oj] >> 5;
 #pragma unroll
                                 for (int q = 0; q < 4; ++q) {
                                     const unsigned o2 = lds_u32(a_Tj + okk[q]);
-                                    pq[q] = (o2 == ROW_NONE) ? nullptr : cell_rows + (o2 + pos[q]);
+                                    pq[q] = (o2 == ROW_NONE) ? ROW_NONE : o2 + pos[q];
                                 }
                             }
                             for (; a + SPU <= run_end; a += SPU) {
