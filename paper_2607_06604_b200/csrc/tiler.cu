@@ -74,7 +74,7 @@ void gr_for_each_tile(gramsci_graph *g, bool need_pix, bool hub_only, gr_tile_fn
     for (auto &w : g->windows) { maxlen = std::max(maxlen, w.e_hi - w.e_lo); maxdense = std::max(maxdense, w.d_hi - w.d_lo); }
     if (!need_dense) maxdense = 0;
     const int K = gr_tiler_slots(g, need_pix, need_dense);
-    if (pair_search && K < 3)
+    if (pair_search && K < std::min(3, W))      // (two windows: every tile touches at most two)
         GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for three windows of %lld edges (4pCF tiles, P:159)", (long long)maxlen);
     if (K < (hub_only ? 1 : 2)) GR_FAIL(GRAMSCI_ENOMEM, "device_mem_cap_bytes too small for two windows of %lld edges", (long long)maxlen);
 

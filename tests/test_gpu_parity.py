@@ -529,7 +529,7 @@ def test_out_of_core_cap_derives_windows():
     assert np.array_equal(g1.pcf4()[0], og.pcf4()[0])      # 4pCF tiles over (h, c1 <= c2)
 
 
-@pytest.mark.parametrize("relabel,n_windows", [(1, 3), (1, 6), (2, 4)])
+@pytest.mark.parametrize("relabel,n_windows", [(1, 2), (1, 3), (1, 6), (2, 4)])
 def test_out_of_core_4pcf_equals_in_core(relabel, n_windows):
     """under a memory cap the 4pCF runs over tiles (hub window h, search windows c1 <= c2); every tetrahedron
     lands in exactly one tile, so counts equal the resident run and the oracle bit for bit (C-13), weighted sums to
