@@ -973,7 +973,7 @@ def test_randomized_shapes_and_options(seed, monkeypatch):
         L = float(rng.choice([20.0, 33.0, 47.0]))
         r_max = float(rng.uniform(2.0, min(8.0, 0.49 * L)))
         r_min = float(rng.choice([0.0, 0.0, rng.uniform(0.0, 0.6 * r_max)]))
-        n = int(min(max(50, float(rng.choice([0.02, 0.08, 0.3])) * L ** 3), 12000))
+        n = int(min(max(50, float(rng.choice([0.02, 0.08, 0.3, 0.6])) * L ** 3), 12000))
         if rng.integers(3) == 0:
             pts = cat.config2_data(seed=int(rng.integers(1 << 30)), n=n, L=L, mean_parents=max(3.0, n / 80.0))["points"]
         else:
@@ -984,12 +984,14 @@ def test_randomized_shapes_and_options(seed, monkeypatch):
             w = w * rng.choice([-1.0, 1.0], n)
         box = [L, L, L] if periodic else None
         og = oracle.Graph(pts, w, box, r_min, r_max, nb)
-        if og.n_edges == 0 or og.n_edges > 4e5:
+        if og.n_edges == 0 or og.n_edges > 1.2e6:
             continue
         algo = int(rng.choice([0, 0, 0, 1, 2, 3]))
-        mode = int(rng.integers(5))
+        mode = int(rng.integers(6))
         for key, val in (("GRAMSCI_FLUSH_BUDGET", str(int(rng.choice([700, 3000, 20000]))) if rng.integers(3) == 0 else None),
-                         ("GRAMSCI_TILE_MB", "1" if rng.integers(4) == 0 else None)):
+                         ("GRAMSCI_TILE_MB", "1" if rng.integers(4) == 0 else None),
+                         ("GRAMSCI_CTA_KMAJOR", str(int(rng.integers(2))) if rng.integers(3) == 0 else None),
+                         ("GRAMSCI_WMODE", "1" if rng.integers(5) == 0 else None)):
             if val is None:
                 monkeypatch.delenv(key, raising=False)
             else:
@@ -1004,6 +1006,8 @@ def test_randomized_shapes_and_options(seed, monkeypatch):
             graphs = [dict(shard_count=k, shard_index=r) for r in range(k)]
         elif mode == 4:
             graphs = [dict(relabel=2)]
+        elif mode == 5:
+            graphs = [dict(want_pixels=True)]
         else:
             graphs = [dict()]
         what = dict(periodic=periodic, nb=nb, L=L, r_min=r_min, r_max=r_max, n=n, weighted=weighted, algo=algo, graphs=graphs)
@@ -1028,6 +1032,14 @@ def test_randomized_shapes_and_options(seed, monkeypatch):
                 c4 += a
                 if weighted:
                     w4 += b
+            if do4 and mode == 5:                                    # parity split: all four channels (A-8 ... A-11)
+                ec, oc, ew, ow = g.pcf4_parity(weighted=weighted)
+                rec, rew, roc, row = og.pcf4(parity=True)
+                assert np.array_equal(ec, rec) and np.array_equal(oc, roc), what
+                if weighted:
+                    sc4 = oracle.Graph(pts, np.abs(w), box, r_min, r_max, nb).pcf4()[1]
+                    assert_weighted_close(ew, rew, scale=sc4)
+                    assert_weighted_close(ow, row, scale=sc4)
             g.free()
         assert mode == 3 or np.array_equal(c2, oc2), what            # (2pCF is not sharded by shard_count)
         assert np.array_equal(c3, oc3), what
