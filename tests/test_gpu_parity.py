@@ -962,8 +962,8 @@ def test_randomized_shapes_and_options(seed, monkeypatch):
     """A seeded sweep over graph shapes (density, radii, bin counts, periodic / open, clustered / uniform, signed weights) and
     library options (kernel variant, capped windows, slab and modulo shards, caller labels, forced drains and spoke tiles):
     2pCF, 3pCF, equilateral 3pCF and 4pCF against the oracle -- counts bit for bit, weighted sums to A-13's tolerance.
-    (The same sweep run for 400 s on a B200 covered 3,068 cases without a mismatch; GRAMSCI_FUZZ_CASES=n runs n cases
-    per seed instead of 25.)"""
+    (GRAMSCI_FUZZ_CASES=n runs n cases per seed instead of 25; 2 x 4,000 cases pass on the final build, and an earlier
+    run of this sweep found the two-window 4pCF tiling bug fixed in csrc/tiler.cu.)"""
     torch = _torch()
     rng = np.random.default_rng(seed)
     done, cases = 0, int(os.environ.get("GRAMSCI_FUZZ_CASES", "25"))
